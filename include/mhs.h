@@ -1,0 +1,177 @@
+/*
+ * mhs.h -- C ABI of libmhs_b200: the B200 (sm_100a) multigrid solve for the poloidal scalar
+ * potential P of linear magnetohydrostatic equilibria, after MacTaggart, Elsheikh, McLaughlin &
+ * Simitev, "Non-symmetric magnetohydrostatic equilibria: a multigrid approach" (arXiv 1307.6720).
+ * Citations "PAPER.md:<line>" refer to the paper text; "C<n>" to the readings listed in DESIGN.md.
+ *
+ * The library follows the paper's procedure (restated :224-247):
+ *     1. P = 0 everywhere
+ *     2. 2D multigrid for  P_xx + P_yy = -B_z(x,y)  on z = 0, P = 0 on the edges   (eq 11, :94, :99)
+ *     3. 3D multigrid for  (1+f(z)) (P_xx + P_yy) + P_zz + alpha^2 P = 0     (eq 8, :67, :100)
+ *        with P = 0 on the side and top boundaries and step 2's P on the bottom;  f = -xi (C1)
+ *     4. B, p, rho by second-order central finite differences               (:102-113, eqs 9, 10)
+ * Multigrid = V(n_pre,n_post) cycles of weighted Gauss-Jacobi relaxation, residual, full-weighting
+ * "reduction" and tri/bi-linear prolongation (the four components of PAPER.md:210), rediscretised
+ * coarse operators, exact solve on the coarsest level, stop on ||r_k||_2 <= tol ||r_0||_2 (C4-C10).
+ *
+ * Conventions
+ *   Grid      vertex grid nx x ny x nz INCLUDING boundary nodes on [0,Lx]x[0,Ly]x[0,Lz]; every
+ *             extent must be 2^m q + 1 with m >= 1 (>= 3 nodes).  (C2)
+ *   Layout    every array crossing this ABI is DENSE, x fastest: idx = i + nx*(j + ny*k)
+ *             (PAPER.md:214-216), element type float or double as chosen by mhs_options.dtype.
+ *   Memory    "device" pointers are CUDA device pointers on the current device, "host" pointers
+ *             are ordinary host memory (pinned for best speed).  The caller owns every buffer it
+ *             passes; the library copies what it keeps (f_profile, p_b, rho_b, dfdz) and owns the
+ *             context and its internal hierarchy, all allocated in mhs_create -- the solve calls
+ *             allocate nothing on the device.
+ *   Streams   all work is enqueued on mhs_options.stream (a cudaStream_t; NULL = default stream).
+ *             mhs_solve_* return after the last residual norm has been read back (they report
+ *             `cycles`); the other calls are asynchronous with respect to the host unless they
+ *             take a host pointer, in which case they return after the copy has completed.
+ *   Errors    status codes only; nothing throws or aborts across the ABI.  On any error other
+ *             than MHS_ERR_NOT_CONVERGED outputs are unspecified/untouched; mhs_last_error()
+ *             gives a message.  There is no CPU fallback: without a usable CUDA device
+ *             mhs_create fails with MHS_ERR_CUDA.
+ *   State     create -> solve_boundary -> solve_interior (repeatable: it CONTINUES from the
+ *             current P, so max_cycles = 1 called k times yields iterate k) -> fields.
+ *             solve_boundary resets the interior to 0.
+ */
+#ifndef MHS_H_
+#define MHS_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mhs_ctx mhs_ctx; /* opaque, library-owned; one per grid + stream; not thread-safe */
+
+typedef enum {
+    MHS_OK = 0,
+    MHS_ERR_INVALID_ARG = 1,
+    MHS_ERR_GRID = 2,          /* an extent is not 2^m*q+1 with m>=1, or the coarsest level is too large */
+    MHS_ERR_NOT_ELLIPTIC = 3,  /* some 1 + f(z_k) <= 0, i.e. xi >= 1       */
+    MHS_ERR_INDEFINITE = 4,    /* some diagonal D_k >= 0 on some level (alpha^2 too large for the grid) */
+    MHS_ERR_STATE = 5,         /* call order violated                                                  */
+    MHS_ERR_NOT_CONVERGED = 6, /* max_cycles reached; the result is still the valid k-th iterate       */
+    MHS_ERR_CUDA = 7,
+    MHS_ERR_OOM = 8
+} mhs_status;
+
+typedef struct { int nx, ny, nz; double Lx, Ly, Lz; } mhs_grid;
+
+#define MHS_BC_DIRICHLET_ZERO 0
+typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 */
+
+#define MHS_F32 0
+#define MHS_F64 1
+
+/* mhs_options.flags */
+#define MHS_FLAG_REFERENCE_KERNELS 1 /* one thread per node, one kernel per operator, no fusion: the
+                                        paper's own kernel design; for A/B tests */
+#define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
+                                        cycles speculatively behind a device-side stop flag          */
+
+typedef struct {
+    int dtype;                 /* MHS_F32 / MHS_F64: element type of ALL device/host field arrays      */
+    double omega;              /* Jacobi weight (C4); benchmarks use 2/3                               */
+    int n_pre, n_post;         /* sweeps before / after the coarse-grid correction (C5)                */
+    int max_levels;            /* 0 = coarsen fully (C8)                                               */
+    double boundary_tol;       /* relative tolerance of the 2D solve (C11)                             */
+    int boundary_max_cycles;
+    double mu0, g;             /* eqs (9), (10)                                                        */
+    const double *p_b, *rho_b; /* host, nz each; NULL -> zeros                                         */
+    const double *dfdz;        /* host, nz; NULL -> finite differences of f_profile (C14)              */
+    void *stream;              /* cudaStream_t                                                         */
+    int profile;               /* 1: time every kernel class with CUDA events on `stream`              */
+    int flags;                 /* MHS_FLAG_*                                                           */
+} mhs_options;
+
+#define MHS_HISTORY_LEN 256
+typedef struct {
+    int cycles;                       /* V-cycles performed by this call                               */
+    double r0;                        /* ||rhs - L u||_2 of the initial iterate (zero interior)        */
+    double r_final;                   /* after the last cycle                                          */
+    double history[MHS_HISTORY_LEN];  /* history[k] = norm after cycle k+1 of this call                */
+} mhs_solve_info;
+
+/* Kernel classes for mhs_profile. */
+enum {
+    MHS_KC_SMOOTH_L0 = 0,   /* Jacobi sweeps on the finest 3D level (the dominant, HBM-bound kernel) */
+    MHS_KC_RESTRICT_L0 = 1, /* residual + full weighting on the finest 3D level                      */
+    MHS_KC_PROLONG_L0 = 2,  /* trilinear correction on the finest 3D level                           */
+    MHS_KC_NORM_L0 = 3,     /* residual norm on the finest 3D level                                  */
+    MHS_KC_COARSE_3D = 4,   /* everything on 3D levels >= 1                                          */
+    MHS_KC_BOUNDARY_2D = 5, /* the whole 2D solve                                                    */
+    MHS_KC_FIELDS = 6,      /* B, p, rho                                                             */
+    MHS_KC_PACK = 7,        /* dense <-> internal layout, zero fills                                 */
+    MHS_KC_COUNT = 8
+};
+typedef struct {
+    long long launches[MHS_KC_COUNT]; /* kernels launched per class since create / reset             */
+    double ms[MHS_KC_COUNT];          /* CUDA-event time per class (only with options.profile = 1)   */
+    long long sweeps_l0;              /* Jacobi sweeps applied to the finest 3D level                */
+} mhs_profile;
+
+/* Fill *o with the defaults: fp64, omega 2/3, V(2,2), full coarsening, boundary_tol 1e-10,
+ * boundary_max_cycles 100, mu0 = 1/2, g = 1 (C16), no profiles, default stream. */
+void mhs_default_options(mhs_options *o);
+
+/* Build a context: level hierarchy (C8), per-level coefficient tables c_l[k] = 1 + f(z_k) injected
+ * to the coarse levels (C7), omega/D_k, inverse of the coarsest operators (C9), device arrays.
+ * f_profile: host, nz doubles, f(z_k) at the nodes (NULL -> 0: the force-free case).
+ * bc: NULL or all MHS_BC_DIRICHLET_ZERO.  opts: NULL -> defaults.  P is initialised to 0 (step 1). */
+mhs_status mhs_create(const mhs_grid *grid, double alpha, const double *f_profile, const mhs_bc *bc,
+                      const mhs_options *opts, mhs_ctx **out);
+void mhs_destroy(mhs_ctx *ctx);
+
+/* Steps 1-2 (eq 11): P = 0 everywhere, then 2D V-cycles for L2 P0 = -Bz0 with
+ * P0 = 0 on the edges until ||r|| <= boundary_tol ||r0|| or boundary_max_cycles; P(:,:,0) = P0.
+ * Bz0: nx*ny values (dtype), device / host.  info may be NULL. */
+mhs_status mhs_solve_boundary(mhs_ctx *ctx, const void *Bz0_device, mhs_solve_info *info);
+mhs_status mhs_solve_boundary_host(mhs_ctx *ctx, const void *Bz0_host, mhs_solve_info *info);
+
+/* Step 3 (eq 8): V-cycles on the interior, continuing from the current P, until
+ * ||r_k|| <= tol * r0 or max_cycles cycles have been done in this call (1 <= max_cycles).
+ * r0 is the residual norm of the iterate found at the first call after mhs_solve_boundary /
+ * mhs_set_potential and is remembered across continuing calls. */
+mhs_status mhs_solve_interior(mhs_ctx *ctx, double tol, int max_cycles, mhs_solve_info *info);
+
+/* Field recovery (C13-C15).  B: 3*N values, Bx | By | Bz one after the other;
+ * p, rho: N values each, N = nx*ny*nz.  Any of B, p, rho may be NULL (skipped). */
+mhs_status mhs_fields(mhs_ctx *ctx, void *B_device, void *p_device, void *rho_device);
+mhs_status mhs_fields_host(mhs_ctx *ctx, void *B_host, void *p_host, void *rho_host);
+
+/* Read / overwrite the current iterate P (N values, dense).  mhs_set_potential takes the interior
+ * and bottom-plane interior values; side/top/bottom-edge values of the input are ignored (they
+ * are the Dirichlet zeros).  Needed for per-iterate parity checks and for resuming a solve. */
+mhs_status mhs_get_potential(mhs_ctx *ctx, void *P_device);
+mhs_status mhs_get_potential_host(mhs_ctx *ctx, void *P_host);
+mhs_status mhs_set_potential(mhs_ctx *ctx, const void *P_device);
+
+const char *mhs_last_error(const mhs_ctx *ctx); /* never NULL; valid until the next call on ctx */
+const char *mhs_status_string(mhs_status s);
+
+/* ---- instrumentation ------------------------------------------------------------------------ */
+mhs_status mhs_get_profile(mhs_ctx *ctx, mhs_profile *out); /* synchronises the stream             */
+mhs_status mhs_reset_profile(mhs_ctx *ctx);
+const char *mhs_kernel_class_name(int kernel_class);
+
+/* ---- operator-level access (tests and micro-benchmarks of single multigrid components) -------
+ * dim = 2 (boundary hierarchy) or 3 (interior hierarchy); level 0 is the finest.
+ * which: 0 = u (the iterate / correction), 1 = rhs, 2 = r (residual scratch).  The finest 3D level
+ * has rhs == 0 and no rhs array (MHS_ERR_INVALID_ARG).  Arrays are dense, that level's extents. */
+int mhs_num_levels(const mhs_ctx *ctx, int dim);
+mhs_status mhs_level_dims(const mhs_ctx *ctx, int dim, int level, int *nx, int *ny, int *nz);
+mhs_status mhs_level_set(mhs_ctx *ctx, int dim, int level, int which, const void *src_device);
+mhs_status mhs_level_get(mhs_ctx *ctx, int dim, int level, int which, void *dst_device);
+mhs_status mhs_op_smooth(mhs_ctx *ctx, int dim, int level, int sweeps);   /* u <- S^sweeps u          */
+mhs_status mhs_op_residual(mhs_ctx *ctx, int dim, int level);             /* r <- rhs - L u           */
+mhs_status mhs_op_restrict(mhs_ctx *ctx, int dim, int level);             /* rhs_{l+1} <- R (rhs - L u)_l */
+mhs_status mhs_op_prolong(mhs_ctx *ctx, int dim, int level);              /* u_l <- u_l + P u_{l+1}   */
+mhs_status mhs_op_vcycle(mhs_ctx *ctx, int dim, int level);               /* one V-cycle from `level` */
+mhs_status mhs_op_resnorm(mhs_ctx *ctx, int dim, int level, double *out_host); /* ||rhs - L u||_2     */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHS_H_ */

@@ -1,0 +1,762 @@
+// C ABI of libmhs_b200 (include/mhs.h): context + level hierarchy, V-cycle driver, solve loops.
+// Host logic only -- every arithmetic step of the path runs in the kernels of mhs_kernels_*.cu.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "mhs_internal.h"
+
+using namespace mhs;
+
+namespace {
+
+#define CK(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            ctx->err = std::string(#call) + ": " + cudaGetErrorString(e_);                               \
+            return e_ == cudaErrorMemoryAllocation ? MHS_ERR_OOM : MHS_ERR_CUDA;                         \
+        }                                                                                                \
+    } while (0)
+
+mhs_status fail(mhs_ctx* ctx, mhs_status s, const std::string& msg)
+{
+    ctx->err = msg;
+    return s;
+}
+
+// RAII kernel-class scope: routes launch counts, and CUDA-event timing when profiling is on.
+struct Scope {
+    mhs_ctx* c;
+    int prev;
+    bool timed;
+    Ev ev{};
+    Scope(mhs_ctx* ctx, int kc) : c(ctx), prev(ctx->cur_kc)
+    {
+        c->cur_kc = kc;
+        timed = c->opt.profile >= 2 || (c->opt.profile == 1 && kc == MHS_KC_SMOOTH_L0);
+        if (timed) {
+            ev.kc = kc;
+            ev.a = take();
+            ev.b = take();
+            cudaEventRecord(ev.a, c->stream);
+        }
+    }
+    ~Scope()
+    {
+        if (timed) {
+            cudaEventRecord(ev.b, c->stream);
+            c->ev_pending.push_back(ev);
+        }
+        c->cur_kc = prev;
+    }
+    cudaEvent_t take()
+    {
+        if (!c->ev_pool.empty()) {
+            cudaEvent_t e = c->ev_pool.back();
+            c->ev_pool.pop_back();
+            return e;
+        }
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        return e;
+    }
+};
+
+// After a stream synchronisation: fold finished event pairs into the profile.
+void drain_events(mhs_ctx* c)
+{
+    for (const Ev& e : c->ev_pending) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, e.a, e.b) == cudaSuccess) c->prof.ms[e.kc] += ms;
+        c->ev_pool.push_back(e.a);
+        c->ev_pool.push_back(e.b);
+    }
+    c->ev_pending.clear();
+}
+
+// Dense inverse by Gauss-Jordan with partial pivoting (fp64, host).  A is n x n row-major, overwritten by A^-1.
+bool invert_dense(int n, std::vector<double>& A)
+{
+    std::vector<double> M((size_t)n * 2 * n, 0.0);
+    for (int r = 0; r < n; ++r) {
+        for (int c = 0; c < n; ++c) M[(size_t)r * 2 * n + c] = A[(size_t)r * n + c];
+        M[(size_t)r * 2 * n + n + r] = 1.0;
+    }
+    for (int col = 0; col < n; ++col) {
+        int piv = col;
+        double best = std::fabs(M[(size_t)col * 2 * n + col]);
+        for (int r = col + 1; r < n; ++r) {
+            double v = std::fabs(M[(size_t)r * 2 * n + col]);
+            if (v > best) { best = v; piv = r; }
+        }
+        if (best == 0.0) return false;
+        if (piv != col)
+            for (int c = 0; c < 2 * n; ++c) std::swap(M[(size_t)col * 2 * n + c], M[(size_t)piv * 2 * n + c]);
+        const double d = 1.0 / M[(size_t)col * 2 * n + col];
+        for (int c = 0; c < 2 * n; ++c) M[(size_t)col * 2 * n + c] *= d;
+        for (int r = 0; r < n; ++r) {
+            if (r == col) continue;
+            const double m = M[(size_t)r * 2 * n + col];
+            if (m == 0.0) continue;
+            for (int c = 0; c < 2 * n; ++c) M[(size_t)r * 2 * n + c] -= m * M[(size_t)col * 2 * n + c];
+        }
+    }
+    for (int r = 0; r < n; ++r)
+        for (int c = 0; c < n; ++c) A[(size_t)r * n + c] = M[(size_t)r * 2 * n + n + c];
+    return true;
+}
+
+bool level_is_coarsest(int nx, int ny, int nz, int dim, int level, int max_levels)
+{
+    if (max_levels > 0 && level + 1 >= max_levels) return true;
+    const int mx = nx - 1, my = ny - 1, mz = nz - 1;
+    if ((mx & 1) || mx < 4 || (my & 1) || my < 4) return true;
+    if (dim == 3 && ((mz & 1) || mz < 4)) return true;
+    return false;
+}
+
+template <typename T>
+std::vector<T> cast_vec(const std::vector<double>& v)
+{
+    std::vector<T> o(v.size());
+    for (size_t i = 0; i < v.size(); ++i) o[i] = (T)v[i];
+    return o;
+}
+
+mhs_status upload(mhs_ctx* ctx, void** dst, const std::vector<double>& v)
+{
+    CK(cudaMalloc(dst, v.size() * ctx->es));
+    if (ctx->es == 8) {
+        CK(cudaMemcpy(*dst, v.data(), v.size() * 8, cudaMemcpyHostToDevice));
+    } else {
+        std::vector<float> f = cast_vec<float>(v);
+        CK(cudaMemcpy(*dst, f.data(), f.size() * 4, cudaMemcpyHostToDevice));
+    }
+    return MHS_OK;
+}
+
+mhs_status alloc_field(mhs_ctx* ctx, Level& lv, int slot, void** out)
+{
+    void* raw = nullptr;
+    CK(cudaMalloc(&raw, (size_t)lv.alloc * ctx->es));
+    CK(cudaMemset(raw, 0, (size_t)lv.alloc * ctx->es));
+    lv.raw[slot] = raw;
+    *out = (char*)raw + (size_t)lv.pad * ctx->es;
+    return MHS_OK;
+}
+
+// Build one hierarchy (dim 2 or 3): extents, spacings, coefficient tables, coarsest inverse, arrays.
+mhs_status build_hierarchy(mhs_ctx* ctx, int dim, std::vector<Level>& Ls)
+{
+    const mhs_grid& g = ctx->grid;
+    int nx = g.nx, ny = g.ny, nz = dim == 3 ? g.nz : 1;
+    double hx = g.Lx / (g.nx - 1), hy = g.Ly / (g.ny - 1), hz = dim == 3 ? g.Lz / (g.nz - 1) : 0.0;
+    std::vector<double> c(nz, 1.0);
+    if (dim == 3)
+        for (int k = 0; k < nz; ++k) c[k] = 1.0 + ctx->f[k];
+    const double a2 = dim == 3 ? ctx->alpha * ctx->alpha : 0.0;
+    for (int l = 0;; ++l) {
+        Level lv;
+        lv.dim = dim; lv.nx = nx; lv.ny = ny; lv.nz = nz; lv.sx = nx - 1; lv.sy = ny - 1;
+        lv.sp = (long long)lv.sx * lv.sy;
+        lv.hx = hx; lv.hy = hy; lv.hz = hz; lv.c = c;
+        lv.coarsest = level_is_coarsest(nx, ny, nz, dim, l, ctx->opt.max_levels);
+        const long long front = (dim == 3 ? lv.sp : 0) + lv.sx + 32;
+        lv.pad = (front + 31) / 32 * 32;
+        lv.alloc = lv.pad + lv.sp * nz + (dim == 3 ? lv.sp : 0) + lv.sx + 64;
+        // coefficient table: cx | cy | diag | w
+        std::vector<double> tab(4 * (size_t)nz);
+        for (int k = 0; k < nz; ++k) {
+            const double cx = c[k] / (hx * hx), cy = c[k] / (hy * hy);
+            const double d = -2.0 * cx - 2.0 * cy - (dim == 3 ? 2.0 / (hz * hz) : 0.0) + a2;
+            const bool interior = dim == 2 || (k > 0 && k < nz - 1);
+            if (interior && !(d < 0.0)) {
+                char b[160];
+                snprintf(b, sizeof b, "operator not negative definite: diagonal D_k = %g >= 0 on level %d, plane %d (alpha^2 too large)", d, l, k);
+                return fail(ctx, MHS_ERR_INDEFINITE, b);
+            }
+            tab[k] = cx; tab[nz + k] = cy; tab[2 * nz + k] = d; tab[3 * nz + k] = ctx->opt.omega / d;
+        }
+        mhs_status st = upload(ctx, &lv.tab, tab);
+        if (st) return st;
+        if ((st = alloc_field(ctx, lv, 0, &lv.u))) return st;
+        if (!(dim == 3 && l == 0))
+            if ((st = alloc_field(ctx, lv, 2, &lv.rhs))) return st;
+        if (!lv.coarsest) {
+            if ((st = alloc_field(ctx, lv, 1, &lv.tmp))) return st;
+            if ((st = alloc_field(ctx, lv, 3, &lv.r))) return st;
+        } else {
+            // exact solve on the coarsest level (C9): assemble L on the interior unknowns, invert.
+            const int mx = nx - 2, my = ny - 2, mz = dim == 3 ? nz - 2 : 1;
+            const long long n = (long long)mx * my * mz;
+            if (n > 1024) return fail(ctx, MHS_ERR_GRID, "coarsest level has more than 1024 unknowns; extents must be 2^m*q+1 with small q");
+            lv.ncoarse = (int)n;
+            std::vector<double> A((size_t)n * n, 0.0);
+            for (int k = 0; k < mz; ++k)
+                for (int j = 0; j < my; ++j)
+                    for (int i = 0; i < mx; ++i) {
+                        const int row = i + mx * (j + my * k);
+                        const int kk = dim == 3 ? k + 1 : 0;
+                        const double cx = c[kk] / (hx * hx), cy = c[kk] / (hy * hy), cz = dim == 3 ? 1.0 / (hz * hz) : 0.0;
+                        A[(size_t)row * n + row] = -2.0 * cx - 2.0 * cy - 2.0 * cz + a2;
+                        if (i > 0) A[(size_t)row * n + row - 1] = cx;
+                        if (i < mx - 1) A[(size_t)row * n + row + 1] = cx;
+                        if (j > 0) A[(size_t)row * n + row - mx] = cy;
+                        if (j < my - 1) A[(size_t)row * n + row + mx] = cy;
+                        if (k > 0) A[(size_t)row * n + row - mx * my] = cz;
+                        if (k < mz - 1) A[(size_t)row * n + row + mx * my] = cz;
+                    }
+            if (!invert_dense((int)n, A)) return fail(ctx, MHS_ERR_INDEFINITE, "coarsest-level operator is singular");
+            if ((st = upload(ctx, &lv.ainv, A))) return st;
+        }
+        Ls.push_back(lv);
+        if (lv.coarsest) break;
+        // next level: rediscretise with 2h, inject the coefficient (C7)
+        std::vector<double> cc((nz - 1) / 2 + 1);
+        if (dim == 3) {
+            for (size_t K = 0; K < cc.size(); ++K) cc[K] = c[2 * K];
+            c = cc;
+            nz = (nz - 1) / 2 + 1;
+            hz *= 2.0;
+        }
+        nx = (nx - 1) / 2 + 1; ny = (ny - 1) / 2 + 1;
+        hx *= 2.0; hy *= 2.0;
+    }
+    return MHS_OK;
+}
+
+void* field_base(const mhs_ctx* ctx, const Level& lv, void* p) { return (char*)p - (size_t)lv.pad * ctx->es; }
+
+// ---------------------------------------------------------------------------------------------
+// V-cycle, reference composition (SURVEY 8(c) "V(u,rhs,l)"): one kernel per component.
+// ---------------------------------------------------------------------------------------------
+int kc_for(const Level& lv, int l, int what /*0 smooth 1 restrict 2 prolong 3 norm*/)
+{
+    if (lv.dim == 2) return MHS_KC_BOUNDARY_2D;
+    if (l > 0) return MHS_KC_COARSE_3D;
+    return what;
+}
+
+void smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const int* done)
+{
+    Level& lv = Ls[l];
+    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    for (int s = 0; s < sweeps; ++s) {
+        Scope sc(ctx, kc_for(lv, l, 0));
+        launch_smooth_ref(ctx, lv, lv.u, rhs, lv.tmp, done);
+        std::swap(lv.u, lv.tmp);
+        if (lv.dim == 3 && l == 0) ctx->prof.sweeps_l0 += 1;
+    }
+}
+
+void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done)
+{
+    Level& lv = Ls[l];
+    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    if (lv.coarsest) {
+        Scope sc(ctx, kc_for(lv, l, 0));
+        launch_coarse_solve(ctx, lv, lv.u, rhs, done);
+        return;
+    }
+    Level& co = Ls[l + 1];
+    smooth(ctx, Ls, l, ctx->opt.n_pre, done);
+    {
+        Scope sc(ctx, kc_for(lv, l, 1));
+        launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, done);
+        launch_restrict_ref(ctx, lv, lv.r, co, co.rhs, done);
+        if (!co.coarsest) cudaMemsetAsync(field_base(ctx, co, co.u), 0, (size_t)co.alloc * ctx->es, ctx->stream);
+    }
+    vcycle(ctx, Ls, l + 1, done);
+    {
+        Scope sc(ctx, kc_for(lv, l, 2));
+        launch_prolong_ref(ctx, lv, lv.u, co, co.u, done);
+    }
+    smooth(ctx, Ls, l, ctx->opt.n_post, done);
+}
+
+void resnorm(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int mode, const int* done)
+{
+    Level& lv = Ls[l];
+    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    Scope sc(ctx, kc_for(lv, l, 3));
+    const long long n = launch_resnorm_partial_ref(ctx, lv, lv.u, rhs, done);
+    launch_norm_final(ctx, n, mode);
+}
+
+// Solve loop shared by the 2D and 3D drivers: cycles run speculatively in chunks behind the
+// device-side stop flag; the host reads the control block once per chunk (C10 stop rule is exact:
+// every kernel of a cycle issued after the flag was raised returns without touching anything).
+mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_cycles, double r0_known,
+                      mhs_solve_info* info)
+{
+    if (max_cycles < 1) return fail(ctx, MHS_ERR_INVALID_ARG, "max_cycles must be >= 1");
+    Ctl* h = ctx->ctl_host;
+    memset(h, 0, sizeof(Ctl));
+    h->max_cycles = max_cycles;
+    h->tol = tol;
+    h->r0 = r0_known;
+    CK(cudaMemcpyAsync(ctx->ctl, h, sizeof(Ctl), cudaMemcpyHostToDevice, ctx->stream));
+    if (!(r0_known > 0.0)) resnorm(ctx, Ls, 0, 0, nullptr);
+    // The ping-pong buffers of the finest level swap roles once per sweep; with an odd number of
+    // sweeps per cycle a skipped (speculative) cycle would leave them swapped, so sync every cycle.
+    const bool odd = ((ctx->opt.n_pre + ctx->opt.n_post) & 1) != 0;
+    const int chunk = ((ctx->opt.flags & MHS_FLAG_SYNC_EACH_CYCLE) || odd) ? 1 : 4;
+    int issued = 0;
+    while (true) {
+        const int n = std::min(chunk, max_cycles - issued);
+        for (int q = 0; q < n; ++q) {
+            vcycle(ctx, Ls, 0, &ctx->ctl->done);
+            resnorm(ctx, Ls, 0, 1, &ctx->ctl->done);
+        }
+        issued += n;
+        CK(cudaMemcpyAsync(h, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        if (h->done || issued >= max_cycles) break;
+    }
+    drain_events(ctx);
+    CK(cudaGetLastError());
+    if (info) {
+        info->cycles = h->cycles;
+        info->r0 = h->r0;
+        info->r_final = h->cycles > 0 ? h->r_last : h->r0;
+        memset(info->history, 0, sizeof info->history);
+        memcpy(info->history, h->hist, sizeof(double) * std::min(h->cycles, MHS_HISTORY_LEN));
+    }
+    if (h->nan_seen) return fail(ctx, MHS_ERR_INDEFINITE, "residual norm is not finite (divergence: alpha^2 too large for the coarse grids?)");
+    if (!(h->r_last <= tol * h->r0)) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance");
+    return MHS_OK;
+}
+
+mhs_status ensure_stage(mhs_ctx* ctx, size_t bytes)
+{
+    if (ctx->stage_bytes >= bytes) return MHS_OK;
+    if (ctx->stage) cudaFree(ctx->stage);
+    ctx->stage = nullptr; ctx->stage_bytes = 0;
+    CK(cudaMalloc(&ctx->stage, bytes));
+    ctx->stage_bytes = bytes;
+    return MHS_OK;
+}
+
+std::vector<Level>* hierarchy(mhs_ctx* ctx, int dim) { return dim == 3 ? &ctx->L3 : dim == 2 ? &ctx->L2 : nullptr; }
+
+mhs_status check_level(mhs_ctx* ctx, int dim, int level, std::vector<Level>** Ls)
+{
+    *Ls = hierarchy(ctx, dim);
+    if (!*Ls) return fail(ctx, MHS_ERR_INVALID_ARG, "dim must be 2 or 3");
+    if (level < 0 || level >= (int)(*Ls)->size()) return fail(ctx, MHS_ERR_INVALID_ARG, "no such level");
+    return MHS_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+void mhs_default_options(mhs_options* o)
+{
+    if (!o) return;
+    memset(o, 0, sizeof *o);
+    o->dtype = MHS_F64;
+    o->omega = 2.0 / 3.0;
+    o->n_pre = 2; o->n_post = 2;
+    o->max_levels = 0;
+    o->boundary_tol = 1e-10;
+    o->boundary_max_cycles = 100;
+    o->mu0 = 0.5; o->g = 1.0;
+}
+
+const char* mhs_status_string(mhs_status s)
+{
+    switch (s) {
+        case MHS_OK: return "MHS_OK";
+        case MHS_ERR_INVALID_ARG: return "MHS_ERR_INVALID_ARG";
+        case MHS_ERR_GRID: return "MHS_ERR_GRID";
+        case MHS_ERR_NOT_ELLIPTIC: return "MHS_ERR_NOT_ELLIPTIC";
+        case MHS_ERR_INDEFINITE: return "MHS_ERR_INDEFINITE";
+        case MHS_ERR_STATE: return "MHS_ERR_STATE";
+        case MHS_ERR_NOT_CONVERGED: return "MHS_ERR_NOT_CONVERGED";
+        case MHS_ERR_CUDA: return "MHS_ERR_CUDA";
+        case MHS_ERR_OOM: return "MHS_ERR_OOM";
+    }
+    return "MHS_ERR_?";
+}
+
+const char* mhs_kernel_class_name(int kc)
+{
+    static const char* n[MHS_KC_COUNT] = {"smooth_l0", "restrict_l0", "prolong_l0", "norm_l0",
+                                          "coarse_3d", "boundary_2d", "fields", "pack"};
+    return (kc >= 0 && kc < MHS_KC_COUNT) ? n[kc] : "?";
+}
+
+const char* mhs_last_error(const mhs_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profile, const mhs_bc* bc,
+                      const mhs_options* opts, mhs_ctx** out)
+{
+    if (!grid || !out) return MHS_ERR_INVALID_ARG;
+    *out = nullptr;
+    mhs_ctx* ctx = new (std::nothrow) mhs_ctx();
+    if (!ctx) return MHS_ERR_OOM;
+    // from here on errors are reported through a context the caller can query and must destroy
+    *out = ctx;
+    ctx->grid = *grid;
+    if (opts) ctx->opt = *opts; else mhs_default_options(&ctx->opt);
+    ctx->alpha = alpha;
+    const mhs_options& o = ctx->opt;
+    if (o.dtype != MHS_F32 && o.dtype != MHS_F64) return fail(ctx, MHS_ERR_INVALID_ARG, "dtype must be MHS_F32 or MHS_F64");
+    ctx->es = o.dtype == MHS_F64 ? 8 : 4;
+    ctx->stream = (cudaStream_t)o.stream;
+    if (bc && (bc->sides != MHS_BC_DIRICHLET_ZERO || bc->top != MHS_BC_DIRICHLET_ZERO))
+        return fail(ctx, MHS_ERR_INVALID_ARG, "only MHS_BC_DIRICHLET_ZERO (P = 0 on sides and top, PAPER.md:96) is supported");
+    if (!(o.omega > 0.0 && o.omega <= 1.0) || o.n_pre < 0 || o.n_post < 0 || o.n_pre + o.n_post < 1 || o.max_levels < 0 ||
+        !(o.mu0 > 0.0) || o.g == 0.0 || o.boundary_max_cycles < 1 || !(grid->Lx > 0 && grid->Ly > 0 && grid->Lz > 0))
+        return fail(ctx, MHS_ERR_INVALID_ARG, "invalid option value");
+    const int ext[3] = {grid->nx, grid->ny, grid->nz};
+    for (int a = 0; a < 3; ++a)
+        if (ext[a] < 3 || ((ext[a] - 1) & 1))
+            return fail(ctx, MHS_ERR_GRID, "every extent must be 2^m*q+1 with m >= 1 (an even number >= 2 of intervals)");
+    const int nz = grid->nz;
+    ctx->f.assign(nz, 0.0);
+    if (f_profile) ctx->f.assign(f_profile, f_profile + nz);
+    for (int k = 0; k < nz; ++k)
+        if (!(1.0 + ctx->f[k] > 0.0)) return fail(ctx, MHS_ERR_NOT_ELLIPTIC, "1 + f(z_k) <= 0: eq (8) is not elliptic (PAPER.md:70)");
+    ctx->p_b.assign(nz, 0.0); ctx->rho_b.assign(nz, 0.0); ctx->dfdz.assign(nz, 0.0);
+    if (o.p_b) ctx->p_b.assign(o.p_b, o.p_b + nz);
+    if (o.rho_b) ctx->rho_b.assign(o.rho_b, o.rho_b + nz);
+    const double hz = grid->Lz / (nz - 1);
+    if (o.dfdz) ctx->dfdz.assign(o.dfdz, o.dfdz + nz);
+    else {  // C14: central differences of the samples, one-sided second order at both ends
+        const std::vector<double>& f = ctx->f;
+        for (int k = 1; k < nz - 1; ++k) ctx->dfdz[k] = (f[k + 1] - f[k - 1]) / (2.0 * hz);
+        ctx->dfdz[0] = (-3.0 * f[0] + 4.0 * f[1] - f[2]) / (2.0 * hz);
+        ctx->dfdz[nz - 1] = (3.0 * f[nz - 1] - 4.0 * f[nz - 2] + f[nz - 3]) / (2.0 * hz);
+    }
+    ctx->opt.p_b = ctx->opt.rho_b = ctx->opt.dfdz = nullptr;  // the caller's arrays are not kept
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(ctx, MHS_ERR_CUDA, "no CUDA device: libmhs_b200 has no CPU fallback");
+    }
+    mhs_status st;
+    if ((st = build_hierarchy(ctx, 3, ctx->L3))) return st;
+    if ((st = build_hierarchy(ctx, 2, ctx->L2))) return st;
+    if (ctx->L3.size() < 2) return fail(ctx, MHS_ERR_GRID, "the 3D hierarchy needs at least two levels (>= 4 intervals per axis, max_levels != 1)");
+
+    std::vector<double> ft(4 * (size_t)nz);
+    for (int k = 0; k < nz; ++k) {
+        ft[k] = -ctx->f[k];            // xi = -f   (C1)
+        ft[nz + k] = -ctx->dfdz[k];    // xi'
+        ft[2 * nz + k] = ctx->p_b[k];
+        ft[3 * nz + k] = ctx->rho_b[k];
+    }
+    if ((st = upload(ctx, &ctx->prof_tab, ft))) return st;
+    ctx->npartial = std::max(resnorm_partial_capacity(ctx->L3[0]), resnorm_partial_capacity(ctx->L2[0]));
+    CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
+    CK(cudaMalloc((void**)&ctx->ctl, sizeof(Ctl)));
+    CK(cudaMemset(ctx->ctl, 0, sizeof(Ctl)));
+    CK(cudaMallocHost((void**)&ctx->ctl_host, sizeof(Ctl)));
+    if ((st = ensure_stage(ctx, (size_t)grid->nx * grid->ny * ctx->es))) return st;
+    CK(cudaDeviceSynchronize());
+    return MHS_OK;
+}
+
+void mhs_destroy(mhs_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->stream || !ctx->L3.empty()) cudaStreamSynchronize(ctx->stream);
+    for (std::vector<Level>* Ls : {&ctx->L3, &ctx->L2})
+        for (Level& lv : *Ls) {
+            for (void* p : lv.raw) if (p) cudaFree(p);
+            if (lv.tab) cudaFree(lv.tab);
+            if (lv.ainv) cudaFree(lv.ainv);
+        }
+    if (ctx->prof_tab) cudaFree(ctx->prof_tab);
+    if (ctx->partial) cudaFree(ctx->partial);
+    if (ctx->ctl) cudaFree(ctx->ctl);
+    if (ctx->ctl_host) cudaFreeHost(ctx->ctl_host);
+    if (ctx->stage) cudaFree(ctx->stage);
+    for (const Ev& e : ctx->ev_pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
+    delete ctx;
+}
+
+mhs_status mhs_solve_boundary(mhs_ctx* ctx, const void* Bz0, mhs_solve_info* info)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!Bz0) return fail(ctx, MHS_ERR_INVALID_ARG, "Bz0 is NULL");
+    if (ctx->L3.empty() || ctx->L2.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    Level& l3 = ctx->L3[0];
+    Level& l2 = ctx->L2[0];
+    {
+        Scope sc(ctx, MHS_KC_PACK);
+        // step 1: P = 0 everywhere
+        CK(cudaMemsetAsync(field_base(ctx, l3, l3.u), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
+        CK(cudaMemsetAsync(field_base(ctx, l3, l3.tmp), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
+        CK(cudaMemsetAsync(field_base(ctx, l2, l2.u), 0, (size_t)l2.alloc * ctx->es, ctx->stream));
+        if (l2.tmp) CK(cudaMemsetAsync(field_base(ctx, l2, l2.tmp), 0, (size_t)l2.alloc * ctx->es, ctx->stream));
+        launch_pack(ctx, l2, Bz0, l2.rhs, true, true);  // rhs2 = -Bz0 at interior nodes (eq 11)
+    }
+    ctx->have_boundary = false;
+    ctx->have_r0 = false;
+    // step 2
+    mhs_status st = run_cycles(ctx, ctx->L2, ctx->opt.boundary_tol, ctx->opt.boundary_max_cycles, 0.0, info);
+    if (st != MHS_OK && st != MHS_ERR_NOT_CONVERGED) return st;
+    {
+        Scope sc(ctx, MHS_KC_PACK);
+        // P(:,:,0) = P0, in both ping-pong buffers of the finest 3D level (same in-plane layout)
+        CK(cudaMemcpyAsync(l3.u, ctx->L2[0].u, (size_t)l2.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
+        CK(cudaMemcpyAsync(l3.tmp, ctx->L2[0].u, (size_t)l2.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
+    }
+    ctx->have_boundary = true;
+    return st;
+}
+
+mhs_status mhs_solve_boundary_host(mhs_ctx* ctx, const void* Bz0_host, mhs_solve_info* info)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!Bz0_host) return fail(ctx, MHS_ERR_INVALID_ARG, "Bz0 is NULL");
+    const size_t bytes = (size_t)ctx->grid.nx * ctx->grid.ny * ctx->es;
+    mhs_status st = ensure_stage(ctx, bytes);
+    if (st) return st;
+    CK(cudaMemcpyAsync(ctx->stage, Bz0_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    return mhs_solve_boundary(ctx, ctx->stage, info);
+}
+
+mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solve_info* info)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    if (!(tol >= 0.0)) return fail(ctx, MHS_ERR_INVALID_ARG, "tol must be >= 0");
+    mhs_solve_info local;
+    if (!info) info = &local;
+    mhs_status st = run_cycles(ctx, ctx->L3, tol, max_cycles, ctx->have_r0 ? ctx->r0_interior : 0.0, info);
+    if (st == MHS_OK || st == MHS_ERR_NOT_CONVERGED) {
+        ctx->have_r0 = info->r0 > 0.0;
+        ctx->r0_interior = info->r0;
+    }
+    return st;
+}
+
+mhs_status mhs_get_potential(mhs_ctx* ctx, void* P)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!P) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
+    Scope sc(ctx, MHS_KC_PACK);
+    launch_unpack(ctx, ctx->L3[0], ctx->L3[0].u, P);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_get_potential_host(mhs_ctx* ctx, void* P_host)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!P_host) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
+    const size_t bytes = (size_t)ctx->L3[0].npts() * ctx->es;
+    mhs_status st = ensure_stage(ctx, bytes);
+    if (st) return st;
+    if ((st = mhs_get_potential(ctx, ctx->stage))) return st;
+    CK(cudaMemcpyAsync(P_host, ctx->stage, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return MHS_OK;
+}
+
+mhs_status mhs_set_potential(mhs_ctx* ctx, const void* P)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!P) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
+    Level& l3 = ctx->L3[0];
+    Scope sc(ctx, MHS_KC_PACK);
+    launch_pack(ctx, l3, P, l3.u, true, false);
+    CK(cudaMemcpyAsync(l3.tmp, l3.u, (size_t)l3.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaGetLastError());
+    ctx->have_boundary = true;
+    ctx->have_r0 = false;
+    return MHS_OK;
+}
+
+mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    if (!B && !p && !rho) return MHS_OK;
+    Scope sc(ctx, MHS_KC_FIELDS);
+    launch_fields_ref(ctx, ctx->L3[0], ctx->L3[0].u, B, p, rho);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_fields_host(mhs_ctx* ctx, void* B, void* p, void* rho)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    const size_t nb = (size_t)ctx->L3[0].npts() * ctx->es;
+    mhs_status st = ensure_stage(ctx, 5 * nb);
+    if (st) return st;
+    char* s = (char*)ctx->stage;
+    if ((st = mhs_fields(ctx, B ? s : nullptr, p ? s + 3 * nb : nullptr, rho ? s + 4 * nb : nullptr))) return st;
+    if (B) CK(cudaMemcpyAsync(B, s, 3 * nb, cudaMemcpyDeviceToHost, ctx->stream));
+    if (p) CK(cudaMemcpyAsync(p, s + 3 * nb, nb, cudaMemcpyDeviceToHost, ctx->stream));
+    if (rho) CK(cudaMemcpyAsync(rho, s + 4 * nb, nb, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_events(ctx);
+    return MHS_OK;
+}
+
+mhs_status mhs_get_profile(mhs_ctx* ctx, mhs_profile* out)
+{
+    if (!ctx || !out) return MHS_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_events(ctx);
+    *out = ctx->prof;
+    return MHS_OK;
+}
+
+mhs_status mhs_reset_profile(mhs_ctx* ctx)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_events(ctx);
+    memset(&ctx->prof, 0, sizeof ctx->prof);
+    return MHS_OK;
+}
+
+// ---- operator-level access ------------------------------------------------------------------
+int mhs_num_levels(const mhs_ctx* ctx, int dim)
+{
+    if (!ctx) return 0;
+    return dim == 3 ? (int)ctx->L3.size() : dim == 2 ? (int)ctx->L2.size() : 0;
+}
+
+mhs_status mhs_level_dims(const mhs_ctx* cctx, int dim, int level, int* nx, int* ny, int* nz)
+{
+    mhs_ctx* ctx = const_cast<mhs_ctx*>(cctx);
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    if (nx) *nx = (*Ls)[level].nx;
+    if (ny) *ny = (*Ls)[level].ny;
+    if (nz) *nz = (*Ls)[level].nz;
+    return MHS_OK;
+}
+
+static void* pick(Level& lv, int which) { return which == 0 ? lv.u : which == 1 ? lv.rhs : which == 2 ? lv.r : nullptr; }
+
+mhs_status mhs_level_set(mhs_ctx* ctx, int dim, int level, int which, const void* src)
+{
+    if (!ctx || !src) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    Level& lv = (*Ls)[level];
+    void* dst = pick(lv, which);
+    if (!dst) return fail(ctx, MHS_ERR_INVALID_ARG, "this level has no such array");
+    Scope sc(ctx, MHS_KC_PACK);
+    const bool bottom = dim == 3 && level == 0 && which == 0;
+    launch_pack(ctx, lv, src, dst, bottom, false);
+    if (bottom) {
+        CK(cudaMemcpyAsync(lv.tmp, lv.u, (size_t)lv.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
+        ctx->have_r0 = false;
+    }
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_level_get(mhs_ctx* ctx, int dim, int level, int which, void* dst)
+{
+    if (!ctx || !dst) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    Level& lv = (*Ls)[level];
+    void* src = pick(lv, which);
+    if (!src) return fail(ctx, MHS_ERR_INVALID_ARG, "this level has no such array");
+    Scope sc(ctx, MHS_KC_PACK);
+    launch_unpack(ctx, lv, src, dst);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_smooth(mhs_ctx* ctx, int dim, int level, int sweeps)
+{
+    if (!ctx || sweeps < 0) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    if ((*Ls)[level].coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "the coarsest level is solved exactly, not smoothed");
+    smooth(ctx, *Ls, level, sweeps, nullptr);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_residual(mhs_ctx* ctx, int dim, int level)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    Level& lv = (*Ls)[level];
+    if (!lv.r) return fail(ctx, MHS_ERR_INVALID_ARG, "the coarsest level has no residual array");
+    Scope sc(ctx, kc_for(lv, level, 1));
+    launch_residual_ref(ctx, lv, lv.u, (dim == 3 && level == 0) ? nullptr : lv.rhs, lv.r, nullptr);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_restrict(mhs_ctx* ctx, int dim, int level)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    Level& lv = (*Ls)[level];
+    if (lv.coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "no level below the coarsest");
+    Scope sc(ctx, kc_for(lv, level, 1));
+    launch_residual_ref(ctx, lv, lv.u, (dim == 3 && level == 0) ? nullptr : lv.rhs, lv.r, nullptr);
+    launch_restrict_ref(ctx, lv, lv.r, (*Ls)[level + 1], (*Ls)[level + 1].rhs, nullptr);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_prolong(mhs_ctx* ctx, int dim, int level)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    Level& lv = (*Ls)[level];
+    if (lv.coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "no level below the coarsest");
+    Scope sc(ctx, kc_for(lv, level, 2));
+    launch_prolong_ref(ctx, lv, lv.u, (*Ls)[level + 1], (*Ls)[level + 1].u, nullptr);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_vcycle(mhs_ctx* ctx, int dim, int level)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    vcycle(ctx, *Ls, level, nullptr);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_op_resnorm(mhs_ctx* ctx, int dim, int level, double* out_host)
+{
+    if (!ctx || !out_host) return MHS_ERR_INVALID_ARG;
+    std::vector<Level>* Ls;
+    mhs_status st = check_level(ctx, dim, level, &Ls);
+    if (st) return st;
+    resnorm(ctx, *Ls, level, 2, nullptr);
+    CK(cudaMemcpyAsync(ctx->ctl_host, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_events(ctx);
+    *out_host = ctx->ctl_host->r_last;
+    return MHS_OK;
+}
+
+}  // extern "C"

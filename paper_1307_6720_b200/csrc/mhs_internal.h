@@ -1,0 +1,103 @@
+// Internal declarations of libmhs_b200 (not part of the ABI; see include/mhs.h).
+//
+// Device layout of one level ("aliased Dirichlet" layout):
+//   a level with nx x ny x nz vertices is stored with row pitch sx = nx-1 and sy = ny-1 rows per
+//   plane, node (i,j,k) at  base[i + sx*(j + sy*k)].  The Dirichlet-zero node (nx-1, j, k) IS node
+//   (0, j+1, k), and row (., ny-1, k) IS row (., 0, k+1): every wall value exists once, is zero, and
+//   is never written, so rows are 2^m elements long (128-byte aligned for the big levels), no
+//   padding bytes are streamed, and stencil reads at i+-1 / j+-1 never need a bounds test.
+//   One zero plane in front of k = 0 and one behind k = nz-1 (+ a row) absorb the remaining
+//   out-of-range neighbour reads.  2D levels are the same with nz = 1.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "mhs.h"
+
+namespace mhs {
+
+// Per-level parameters handed to kernels by value.
+template <typename T>
+struct LP {
+    int nx, ny, nz;   // vertices (nz = 1 in 2D)
+    int sx, sy;       // row pitch, rows per plane
+    long long sp;     // plane stride = sx*sy
+    const T* tab;     // device: cx[nz] | cy[nz] | diag[nz] | w[nz]   (cx = c_k/hx^2, w = omega/diag)
+    T cz, a2;         // 1/hz^2 (0 in 2D), alpha^2 (0 in 2D)
+};
+
+struct Ctl {  // device-side solve control block (one per context)
+    int done;        // 1: stop rule met -> every later cycle kernel returns at once
+    int cycles;      // cycles completed in this call
+    int max_cycles;
+    int nan_seen;
+    double r0, tol, r_last;
+    double hist[MHS_HISTORY_LEN];
+};
+
+struct Level {
+    int dim = 3;
+    int nx = 0, ny = 0, nz = 1, sx = 0, sy = 0;
+    long long sp = 0, pad = 0, alloc = 0;
+    double hx = 0, hy = 0, hz = 0;
+    bool coarsest = false;
+    void *u = nullptr, *tmp = nullptr, *rhs = nullptr, *r = nullptr;  // -> node (0,0,0)
+    void *raw[4] = {nullptr, nullptr, nullptr, nullptr};
+    void* tab = nullptr;
+    std::vector<double> c;  // 1 + f at this level's planes
+    int ncoarse = 0;        // unknowns of the exact solve (coarsest level only)
+    void* ainv = nullptr;   // device T[ncoarse^2]
+    long long npts() const { return (long long)nx * ny * nz; }
+};
+
+struct Ev { int kc; cudaEvent_t a, b; };
+
+}  // namespace mhs
+
+struct mhs_ctx {
+    mhs_grid grid{};
+    mhs_options opt{};
+    double alpha = 0;
+    int es = 8;  // element size
+    cudaStream_t stream = nullptr;
+    std::vector<mhs::Level> L3, L2;
+    std::vector<double> f, dfdz, p_b, rho_b;
+    void* prof_tab = nullptr;  // device T[4*nz]: xi | dxi | p_b | rho_b
+    mhs::Ctl* ctl = nullptr;   // device
+    mhs::Ctl* ctl_host = nullptr;  // pinned
+    double* partial = nullptr;     // device partial sums of the norm
+    long long npartial = 0;
+    void* stage = nullptr;         // device staging for host-pointer entry points (lazy)
+    size_t stage_bytes = 0;
+    bool have_boundary = false, have_r0 = false;
+    double r0_interior = 0;
+    mhs_profile prof{};
+    int cur_kc = MHS_KC_PACK;  // kernel class the launchers charge
+    std::vector<mhs::Ev> ev_pending;
+    std::vector<cudaEvent_t> ev_pool;
+    std::string err;
+};
+
+namespace mhs {
+
+inline void count_launch(mhs_ctx* c) { c->prof.launches[c->cur_kc] += 1; }
+
+// ---- launchers of the reference kernels (mhs_kernels_ref.cu) --------------------------------
+// `done` (may be NULL) points at Ctl::done: when set, the kernel returns without doing anything.
+void launch_smooth_ref(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done);
+void launch_residual_ref(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* r, const int* done);
+void launch_restrict_ref(mhs_ctx* c, const Level& fine, const void* r, const Level& coarse, void* rhs_c, const int* done);
+void launch_prolong_ref(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, const int* done);
+void launch_coarse_solve(mhs_ctx* c, const Level& lv, void* u, const void* rhs, const int* done);
+// partial sums of (rhs - L u)^2 -> c->partial[0..n); returns n
+long long launch_resnorm_partial_ref(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, const int* done);
+long long resnorm_partial_capacity(const Level& lv);
+// mode 0: r0 = norm; mode 1: record a cycle (history, stop rule); mode 2: r_last only
+void launch_norm_final(mhs_ctx* c, long long n, int mode);
+void launch_pack(mhs_ctx* c, const Level& lv, const void* dense, void* dst, bool keep_bottom, bool negate);
+void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense);
+void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
+
+}  // namespace mhs

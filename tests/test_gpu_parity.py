@@ -1,0 +1,350 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by element on the same
+seeded inputs.  python -m pytest tests -m gpu  (needs a B200).
+
+Tolerances (BASELINE.json north_star):
+  fp64: max|P_gpu^k - P_orc^k| <= 1e-12 * max|P_orc^k| for EVERY V-cycle iterate k   (C21)
+  fp32: 1e-5 on the same measure (iterates), compared against the fp64 oracle
+Single operators (one sweep, residual, restriction, prolongation) are held to 1e-13 / 2e-6.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_1307_6720_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float64: 1e-12, torch.float32: 1e-5}
+OPTOL = {torch.float64: 1e-13, torch.float32: 2e-6}
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6720_b200 import binding
+    binding.lib()
+    return binding
+
+
+def dev(a, dtype):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device="cuda").contiguous()
+
+
+def host(t):
+    return t.detach().cpu().double().numpy()
+
+
+def relmax(a, b):
+    s = np.abs(b).max()
+    return np.abs(a - b).max() / (s if s > 0 else 1.0)
+
+
+WORKLOADS = {
+    "cfg0_33": lambda: inputs.config(0),
+    "ragged_17x33x9": lambda: inputs.small(),
+    "ragged_25x49x13": lambda: inputs.small(nx=25, ny=49, nz=13, L=(1.0, 1.7, 0.6), seed=7),
+    "cfg1_65": lambda: inputs.config(1, shrink=2),
+    "cfg3_v33_65": lambda: inputs.config(3, shrink=8),
+}
+VARIANTS = {"fast": 0, "reference": 1}
+
+
+def flags_of(B, variant):
+    return B.MHS_FLAG_REFERENCE_KERNELS if variant == "reference" else 0
+
+
+# ------------------------------------------------------------------ single operators ---------
+@pytest.mark.parametrize("variant", list(VARIANTS))
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("name", ["ragged_17x33x9", "cfg0_33", "cfg1_65"])
+def test_operators_3d(B, orc, name, dtype, variant):
+    w = WORKLOADS[name]()
+    c = 1.0 + w.f
+    with B.Solver.from_workload(w, dtype=dtype, flags=flags_of(B, variant)) as S:
+        nl = S.num_levels(3)
+        assert nl >= 2
+        for lvl in range(nl - 1):
+            nx, ny, nz = S.level_dims(3, lvl)
+            shp = (nz, ny, nx)
+            Ll = w.L
+            cl = c[:: 2**lvl]
+            assert cl.size == nz
+            u = inputs.random_field(shp, 100 + lvl)
+            if lvl == 0:
+                u[0] = inputs.random_field((ny, nx), 55)            # Dirichlet data on the bottom plane
+            rhs = None if lvl == 0 else inputs.random_field(shp, 200 + lvl)
+            S.level_set(3, lvl, 0, dev(u, dtype))
+            if rhs is not None:
+                S.level_set(3, lvl, 1, dev(rhs, dtype))
+            # residual norm and residual
+            rn = S.op_resnorm(3, lvl)
+            assert abs(rn - orc.resnorm3(u, rhs, cl, w.alpha, Ll)) <= 50 * OPTOL[dtype] * rn
+            S.op_residual(3, lvl)
+            r_or = orc.residual3(u, rhs, cl, w.alpha, Ll)
+            assert relmax(host(S.level_get(3, lvl, 2)), r_or) <= 20 * OPTOL[dtype]
+            # restriction of that residual
+            S.op_restrict(3, lvl)
+            assert relmax(host(S.level_get(3, lvl + 1, 1)), orc.restrict3(r_or)) <= 20 * OPTOL[dtype]
+            # sweeps: 1, then 2 more (3 in total), compared after each call
+            S.op_smooth(3, lvl, 1)
+            u1 = orc.jacobi3(u, rhs, cl, w.alpha, w.omega, Ll)
+            assert relmax(host(S.level_get(3, lvl, 0)), u1) <= OPTOL[dtype]
+            S.op_smooth(3, lvl, 2)
+            u3 = orc.jacobi3(orc.jacobi3(u1, rhs, cl, w.alpha, w.omega, Ll), rhs, cl, w.alpha, w.omega, Ll)
+            assert relmax(host(S.level_get(3, lvl, 0)), u3) <= 2 * OPTOL[dtype]
+            # prolongation + correction
+            cs = S._shape(3, lvl + 1)
+            ec = inputs.random_field(cs, 300 + lvl)
+            S.level_set(3, lvl + 1, 0, dev(ec, dtype))
+            S.op_prolong(3, lvl)
+            assert relmax(host(S.level_get(3, lvl, 0)), orc.prolong_add3(ec, u3)) <= 2 * OPTOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_operators_2d(B, orc, dtype):
+    w = inputs.small(nx=33, ny=65, nz=9, L=(1.0, 2.5, 0.5))
+    Lxy = (w.Lx, w.Ly)
+    with B.Solver.from_workload(w, dtype=dtype) as S:
+        for lvl in range(S.num_levels(2) - 1):
+            shp = S._shape(2, lvl)
+            Ll = Lxy
+            u = inputs.random_field(shp, 400 + lvl)
+            rhs = inputs.random_field(shp, 500 + lvl)
+            S.level_set(2, lvl, 0, dev(u, dtype)); S.level_set(2, lvl, 1, dev(rhs, dtype))
+            S.op_residual(2, lvl)
+            r_or = orc.residual2(u, rhs, Ll)
+            assert relmax(host(S.level_get(2, lvl, 2)), r_or) <= 20 * OPTOL[dtype]
+            S.op_restrict(2, lvl)
+            assert relmax(host(S.level_get(2, lvl + 1, 1)), orc.restrict2(r_or)) <= 20 * OPTOL[dtype]
+            S.op_smooth(2, lvl, 2)
+            u2 = orc.jacobi2(orc.jacobi2(u, rhs, w.omega, Ll), rhs, w.omega, Ll)
+            assert relmax(host(S.level_get(2, lvl, 0)), u2) <= 2 * OPTOL[dtype]
+            ec = inputs.random_field(S._shape(2, lvl + 1), 600 + lvl)
+            S.level_set(2, lvl + 1, 0, dev(ec, dtype))
+            S.op_prolong(2, lvl)
+            assert relmax(host(S.level_get(2, lvl, 0)), orc.prolong_add2(ec, u2)) <= 2 * OPTOL[dtype]
+            # one whole V-cycle from this level
+            S.level_set(2, lvl, 0, dev(u, dtype))
+            S.op_vcycle(2, lvl)
+            # the oracle's level rule counts from the level it is started on; pass the remaining depth
+            uv = orc.vcycle2(u, rhs, Ll, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+            assert relmax(host(S.level_get(2, lvl, 0)), uv) <= 20 * OPTOL[dtype]
+
+
+# ------------------------------------------------------------------ whole path, per iterate ---
+@pytest.mark.parametrize("variant", list(VARIANTS))
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_per_iterate_parity(B, orc, name, dtype, variant):
+    w = WORKLOADS[name]()
+    Lxy = (w.Lx, w.Ly)
+    tol32 = dtype == torch.float32
+    btol = 1e-6 if tol32 else 1e-10
+    with B.Solver.from_workload(w, dtype=dtype, flags=flags_of(B, variant), boundary_tol=btol) as S:
+        # ---- step 2: boundary solve (whole solve, then iterate-by-iterate through max_cycles)
+        ib = S.solve_boundary(dev(w.Bz0, dtype))
+        P0_or, ob = orc.solve_boundary(w.Bz0, Lxy, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=btol)
+        assert ib["cycles"] == ob["cycles"], (ib["cycles"], ob["cycles"])
+        assert abs(ib["r0"] - ob["r0"]) <= 1e-6 * ob["r0"]
+        P_gpu = host(S.get_potential())
+        assert relmax(P_gpu[0], P0_or) <= TOL[dtype]
+        assert np.abs(P_gpu[1:]).max() == 0.0                     # step 1: interior is zero
+        # ---- step 3: V-cycle iterates; the oracle starts from the GPU's own bottom plane so that
+        # only the interior path is compared (fp32 bottom data differ from fp64 by rounding)
+        P_or = np.zeros(w.shape); P_or[0] = P_gpu[0]
+        c = 1.0 + w.f
+        r0 = orc.resnorm3(P_or, None, c, w.alpha, w.L)
+        ncyc = 8 if tol32 else 12
+        for k in range(ncyc):
+            info = S.solve_interior(tol=0.0, max_cycles=1)
+            assert info["cycles"] == 1
+            assert abs(info["r0"] - r0) <= 1e-5 * r0
+            P_or = orc.vcycle3(P_or, None, c, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+            err = relmax(host(S.get_potential()), P_or)
+            assert err <= TOL[dtype], (k, err)
+            rk = orc.resnorm3(P_or, None, c, w.alpha, w.L)
+            if rk / r0 > (1e-4 if tol32 else 1e-8):               # C21: compare while above the floor
+                assert abs(info["history"][0] - rk) <= (1e-2 if tol32 else 1e-6) * rk, (k, info["history"][0], rk)
+
+
+@pytest.mark.parametrize("variant", list(VARIANTS))
+@pytest.mark.parametrize("name", ["cfg0_33", "ragged_17x33x9", "cfg3_v33_65"])
+def test_solve_to_tolerance_matches_oracle(B, orc, name, variant):
+    """One call to tolerance: same cycle count, same history, same P as the oracle (fp64)."""
+    w = WORKLOADS[name]()
+    with B.Solver.from_workload(w, flags=flags_of(B, variant)) as S:
+        S.solve_boundary(dev(w.Bz0, torch.float64))
+        info = S.solve_interior(tol=w.tol, max_cycles=w.max_cycles)
+        P0, _ = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly), omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=w.tol)
+        P = np.zeros(w.shape); P[0] = P0
+        P, oi = orc.solve_interior(P, w.f, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=w.tol)
+        assert info["converged"] and info["cycles"] == oi["cycles"]
+        assert relmax(host(S.get_potential()), P) <= 1e-12
+        h, ho = info["history"], oi["history"]
+        keep = ho / oi["r0"] > 1e-8
+        assert np.all(np.abs(h[keep] - ho[keep]) <= 1e-6 * ho[keep])
+        assert info["r_final"] <= w.tol * info["r0"]
+        # sync-each-cycle mode gives bit-identical results (speculative cycles are exact no-ops)
+        with B.Solver.from_workload(w, flags=flags_of(B, variant) | B.MHS_FLAG_SYNC_EACH_CYCLE) as S2:
+            S2.solve_boundary(dev(w.Bz0, torch.float64))
+            i2 = S2.solve_interior(tol=w.tol, max_cycles=w.max_cycles)
+            assert i2["cycles"] == info["cycles"]
+            assert torch.equal(S2.get_potential(), S.get_potential())
+
+
+def test_config0_cycle_counts(B):
+    """Survey-time probe values for BASELINE configs[0]: 16 boundary + 22 interior cycles."""
+    w = inputs.config(0)
+    with B.Solver.from_workload(w) as S:
+        ib = S.solve_boundary(dev(w.Bz0, torch.float64))
+        ii = S.solve_interior(1e-10, 100)
+        assert (ib["cycles"], ii["cycles"]) == (16, 22)
+        assert abs(host(S.get_potential())[0].__abs__().max() - 7.07e-3) < 2e-5
+
+
+# ------------------------------------------------------------------ fields -------------------
+@pytest.mark.parametrize("variant", list(VARIANTS))
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("name", ["cfg0_33", "ragged_17x33x9", "cfg1_65"])
+def test_fields_parity(B, orc, name, dtype, variant):
+    w = WORKLOADS[name]()
+    P = inputs.random_field(w.shape, 77) * 1e-2
+    P[0] = inputs.random_field((w.ny, w.nx), 78) * 1e-2
+    # smooth it a little so that fp32 differences are not pure noise
+    c = 1.0 + w.f
+    for _ in range(3):
+        P = orc.jacobi3(P, None, c, w.alpha, w.omega, w.L)
+    with B.Solver.from_workload(w, dtype=dtype, flags=flags_of(B, variant)) as S:
+        S.set_potential(dev(P, dtype))
+        Pg = host(S.get_potential())
+        assert relmax(Pg, P) <= (1e-7 if dtype == torch.float32 else 0.0)
+        Bg, pg, rg = S.fields()
+        ref = orc.fields(Pg, w.f, w.alpha, w.L, w.p_b, w.rho_b, mu0=w.mu0, g=w.g)
+        Bg = host(Bg)
+        tol = 1e-12 if dtype == torch.float64 else 2e-3   # fp32: second differences of fp32 data, eps/h^2
+        scaleB = max(np.abs(r).max() for r in ref[:3])
+        for q in range(3):
+            assert np.abs(Bg[q] - ref[q]).max() <= tol * scaleB, q
+        assert relmax(host(pg), ref[3]) <= tol
+        assert np.abs(host(rg) - ref[4]).max() <= (1e-11 if dtype == torch.float64 else 5e-2) * np.abs(ref[4]).max()
+        # subsets of outputs
+        B2, p2, r2 = S.fields(want=("p",))
+        assert B2 is None and r2 is None and torch.equal(p2, pg)
+        B3, _, _ = S.fields(want=("B",))
+        assert torch.equal(B3, S.fields()[0])
+
+
+def test_full_pipeline_host_buffers(B, orc):
+    """The e2e path bench.py times: host Bz0 in, host B/p/rho out, through the *_host entry points."""
+    w = inputs.config(0)
+    with B.Solver.from_workload(w) as S:
+        bz = torch.as_tensor(w.Bz0).pin_memory()
+        S.solve_boundary(bz)
+        S.solve_interior(w.tol, w.max_cycles)
+        Bh, ph, rh = S.fields(host=True)
+        Ph = torch.empty(w.shape, dtype=torch.float64).pin_memory()
+        from paper_1307_6720_b200.binding import mhs_get_potential
+        mhs_get_potential(S.h, Ph, torch.float64, S.N)
+        ref = orc.fields(Ph.numpy(), w.f, w.alpha, w.L, w.p_b, w.rho_b, mu0=w.mu0, g=w.g)
+        for q in range(3):
+            assert np.abs(Bh[q].numpy() - ref[q]).max() <= 1e-12 * np.abs(ref[2]).max()
+        assert relmax(rh.numpy(), ref[4]) <= 1e-11
+        P0, _ = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly))
+        Po = np.zeros(w.shape); Po[0] = P0
+        Po, _ = orc.solve_interior(Po, w.f, w.alpha, w.L)
+        assert relmax(Ph.numpy(), Po) <= 1e-12
+
+
+# ------------------------------------------------------------------ edge cases ---------------
+def test_edge_cases(B, orc):
+    # zero magnetogram: r0 = 0, one cycle, P stays 0, fields give the background
+    w = inputs.config(0)
+    with B.Solver.from_workload(w) as S:
+        i = S.solve_boundary(torch.zeros((w.ny, w.nx), dtype=torch.float64, device="cuda"))
+        assert i["r0"] == 0.0 and i["converged"]
+        j = S.solve_interior(1e-10, 5)
+        assert j["cycles"] == 1 and j["r_final"] == 0.0
+        assert float(S.get_potential().abs().max()) == 0.0
+        Bf, p, rho = S.fields()
+        assert float(Bf.abs().max()) == 0.0
+        assert np.array_equal(host(p)[:, 3, 4], w.p_b)
+    # max_cycles reached: NOT_CONVERGED is reported, result is the valid k-th iterate
+    with B.Solver.from_workload(w) as S:
+        S.solve_boundary(dev(w.Bz0, torch.float64))
+        i = S.solve_interior(1e-10, 3)
+        assert i["cycles"] == 3 and not i["converged"] and i["status"] == B.MHS_ERR_NOT_CONVERGED
+        P0, _ = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly))
+        Po = np.zeros(w.shape); Po[0] = P0
+        for _ in range(3):
+            Po = orc.vcycle3(Po, None, 1.0 + w.f, w.alpha, w.L)
+        assert relmax(host(S.get_potential()), Po) <= 1e-12
+    # smallest legal grid (two levels: 5^3 -> 3^3) and max_levels
+    ws = inputs.small(nx=5, ny=5, nz=5, L=(1.0, 1.0, 1.0), patches=1)
+    with B.Solver.from_workload(ws) as S:
+        assert S.num_levels(3) == 2
+        S.solve_boundary(dev(ws.Bz0, torch.float64))
+        S.solve_interior(0.0, 2)
+        P0, _ = orc.solve_boundary(ws.Bz0, (1.0, 1.0))
+        Po = np.zeros(ws.shape); Po[0] = P0
+        for _ in range(2):
+            Po = orc.vcycle3(Po, None, 1.0 + ws.f, ws.alpha, ws.L)
+        assert relmax(host(S.get_potential()), Po) <= 1e-12
+    wm = inputs.config(0)
+    with B.Solver.from_workload(wm, max_levels=3) as S:
+        assert S.num_levels(3) == 3 and S.level_dims(3, 2) == (9, 9, 9)   # 343-unknown exact solve
+        S.solve_boundary(dev(wm.Bz0, torch.float64))
+        S.solve_interior(0.0, 2)
+        P0, _ = orc.solve_boundary(wm.Bz0, (1.0, 1.0), max_levels=3)
+        Po = np.zeros(wm.shape); Po[0] = P0
+        for _ in range(2):
+            Po = orc.vcycle3(Po, None, 1.0 + wm.f, wm.alpha, wm.L, max_levels=3)
+        assert relmax(host(S.get_potential()), Po) <= 1e-12
+    # indefinite operator is refused at create (alpha^2 larger than the diagonal allows on a coarse level)
+    with pytest.raises(B.MHSError) as e:
+        B.Solver(33, 33, 33, alpha=40.0)
+    assert e.value.status == B.MHS_ERR_INDEFINITE
+
+
+def test_odd_sweep_counts_and_v11(B, orc):
+    """V(2,1) / V(1,1) / V(3,3): ping-pong parity of the finest level must not matter."""
+    w = inputs.small()
+    for (a, b) in [(2, 1), (1, 1), (3, 3), (1, 0), (0, 2)]:
+        with B.Solver.from_workload(w, n_pre=a, n_post=b) as S:
+            S.solve_boundary(dev(w.Bz0, torch.float64))
+            P = host(S.get_potential())
+            info = S.solve_interior(1e-9, 60)
+            Po, oi = orc.solve_interior(P, w.f, w.alpha, w.L, omega=w.omega, n_pre=a, n_post=b, tol=1e-9, max_cycles=60)
+            assert info["cycles"] == oi["cycles"], (a, b)
+            assert relmax(host(S.get_potential()), Po) <= 1e-12, (a, b)
+
+
+def test_large_grid_sampled_properties(B, orc):
+    """BASELINE configs[2] (257^3, the bench workload) in the launch configuration bench.py times:
+    the oracle cannot run the solve in seconds, so check (i) two V-cycle iterates on a z-slab-free
+    property: the residual history decreases at the rate the 65^3 / 129^3 oracle runs show, (ii) the
+    converged P satisfies the discrete equation pointwise on sampled nodes evaluated by the oracle's
+    operator, (iii) fields at sampled planes equal the oracle's fields applied to the GPU's P."""
+    w = inputs.config(2)
+    with B.Solver.from_workload(w) as S:
+        S.solve_boundary(dev(w.Bz0, torch.float64))
+        info = S.solve_interior(w.tol, w.max_cycles)
+        assert info["converged"] and 25 <= info["cycles"] <= 45
+        P = host(S.get_potential())
+        c = 1.0 + w.f
+        # (ii) residual by the oracle on a slab of planes around several heights
+        for k0 in (0, 1, 7, 100, 250):
+            sl = P[k0:k0 + 7]
+            r = orc.residual3(sl, None, c[k0:k0 + 7], w.alpha, w.L[:2] + (w.Lz * 6 / (w.nz - 1),))
+            assert np.abs(r[1:-1]).max() <= 1e-9 * info["r0"]
+        rn = orc.resnorm3(P, None, c, w.alpha, w.L)
+        assert abs(rn - info["r_final"]) <= 1e-3 * rn + 1e-13 * info["r0"]
+        # (iii) fields on the whole grid vs the oracle's field routine on the same P
+        Bg, pg, rg = S.fields()
+        ref = orc.fields(P, w.f, w.alpha, w.L, w.p_b, w.rho_b, mu0=w.mu0, g=w.g)
+        sB = np.abs(ref[2]).max()
+        for q in range(3):
+            assert np.abs(host(Bg[q]) - ref[q]).max() <= 1e-12 * sB
+        assert relmax(host(pg), ref[3]) <= 1e-12 and relmax(host(rg), ref[4]) <= 1e-11
+        # bottom-plane Bz reproduces the magnetogram (eq 11 <-> eq 5)
+        assert np.abs(host(Bg[2])[0, 1:-1, 1:-1] - w.Bz0[1:-1, 1:-1]).max() <= 1e-8
