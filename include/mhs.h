@@ -92,6 +92,8 @@ typedef struct {
     double r0;                        /* ||rhs - L u||_2 of the initial iterate (zero interior)        */
     double r_final;                   /* after the last cycle                                          */
     double history[MHS_HISTORY_LEN];  /* history[k] = norm after cycle k+1 of this call                */
+    int stagnated;                    /* fp32 only (C20): stopped because r_k > 0.9 r_{k-1} twice in a
+                                         row -- the fp32 residual floor; reported as MHS_OK          */
 } mhs_solve_info;
 
 /* Kernel classes for mhs_profile. */

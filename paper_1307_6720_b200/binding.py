@@ -53,7 +53,7 @@ class mhs_options(C.Structure):
 
 class mhs_solve_info(C.Structure):
     _fields_ = [("cycles", C.c_int), ("r0", C.c_double), ("r_final", C.c_double),
-                ("history", C.c_double * MHS_HISTORY_LEN)]
+                ("history", C.c_double * MHS_HISTORY_LEN), ("stagnated", C.c_int)]
 
 
 class mhs_profile(C.Structure):
@@ -146,7 +146,8 @@ def _hd(a):
 def _info(i: mhs_solve_info, status):
     n = min(i.cycles, MHS_HISTORY_LEN)
     return dict(cycles=i.cycles, r0=i.r0, r_final=i.r_final, history=np.array(i.history[:n]),
-                converged=status == MHS_OK, status=status)
+                converged=status == MHS_OK, status=status,
+                stagnated=bool(i.stagnated))
 
 
 # ------------------------------------------------------------------ C-named functions ---------

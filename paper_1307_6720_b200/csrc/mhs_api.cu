@@ -297,6 +297,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
     h->max_cycles = max_cycles;
     h->tol = tol;
     h->r0 = r0_known;
+    h->stag_on = ctx->es == 4;
     CK(cudaMemcpyAsync(ctx->ctl, h, sizeof(Ctl), cudaMemcpyHostToDevice, ctx->stream));
     if (!(r0_known > 0.0)) resnorm(ctx, Ls, 0, 0, nullptr);
     // The ping-pong buffers of the finest level swap roles once per sweep; with an odd number of
@@ -321,11 +322,12 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
         info->cycles = h->cycles;
         info->r0 = h->r0;
         info->r_final = h->cycles > 0 ? h->r_last : h->r0;
+        info->stagnated = h->stagnated;
         memset(info->history, 0, sizeof info->history);
         memcpy(info->history, h->hist, sizeof(double) * std::min(h->cycles, MHS_HISTORY_LEN));
     }
     if (h->nan_seen) return fail(ctx, MHS_ERR_INDEFINITE, "residual norm is not finite (divergence: alpha^2 too large for the coarse grids?)");
-    if (!(h->r_last <= tol * h->r0)) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance");
+    if (!(h->r_last <= tol * h->r0) && !h->stagnated) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance");
     return MHS_OK;
 }
 

@@ -33,6 +33,7 @@ struct Ctl {  // device-side solve control block (one per context)
     int cycles;      // cycles completed in this call
     int max_cycles;
     int nan_seen;
+    int stag_on, stag_count, stagnated, pad_;  // fp32 stagnation rule (C20)
     double r0, tol, r_last;
     double hist[MHS_HISTORY_LEN];
 };

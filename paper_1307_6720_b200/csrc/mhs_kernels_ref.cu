@@ -145,12 +145,19 @@ __global__ void __launch_bounds__(1024) k_norm_final(const double* __restrict__ 
             ctl->r0 = r;
         } else if (mode == 1) {
             const int k = ctl->cycles;
+            const double prev = k > 0 ? ctl->r_last : ctl->r0;
             if (k < MHS_HISTORY_LEN) ctl->hist[k] = r;
             ctl->cycles = k + 1;
             ctl->r_last = r;
             const bool bad = !(r == r) || isinf(r);
             if (bad) ctl->nan_seen = 1;
-            if (bad || r <= ctl->tol * ctl->r0 || k + 1 >= ctl->max_cycles) ctl->done = 1;
+            bool stag = false;
+            if (ctl->stag_on) {  // C20: the fp32 residual floor shows as r_k > 0.9 r_{k-1} twice in a row
+                ctl->stag_count = (r > 0.9 * prev) ? ctl->stag_count + 1 : 0;
+                stag = ctl->stag_count >= 2;
+                if (stag) ctl->stagnated = 1;
+            }
+            if (bad || stag || r <= ctl->tol * ctl->r0 || k + 1 >= ctl->max_cycles) ctl->done = 1;
         } else {
             ctl->r_last = r;
         }

@@ -145,7 +145,11 @@ def test_per_iterate_parity(B, orc, name, dtype, variant):
         # ---- step 2: boundary solve (whole solve, then iterate-by-iterate through max_cycles)
         ib = S.solve_boundary(dev(w.Bz0, dtype))
         P0_or, ob = orc.solve_boundary(w.Bz0, Lxy, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=btol)
-        assert ib["cycles"] == ob["cycles"], (ib["cycles"], ob["cycles"])
+        if tol32:   # fp32 stops at 1e-6 or on the stagnation rule (C20); compare with the converged oracle
+            assert ib["converged"] and (ib["stagnated"] or ib["r_final"] <= btol * ib["r0"])
+            P0_or, ob = orc.solve_boundary(w.Bz0, Lxy, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=1e-10)
+        else:
+            assert ib["cycles"] == ob["cycles"], (ib["cycles"], ob["cycles"])
         assert abs(ib["r0"] - ob["r0"]) <= 1e-6 * ob["r0"]
         P_gpu = host(S.get_potential())
         assert relmax(P_gpu[0], P0_or) <= TOL[dtype]
