@@ -1,0 +1,276 @@
+#!/usr/bin/env python
+"""bench.py -- V-cycles/s and smoother HBM GB/s of the MHS multigrid hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config I]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path over one synthetic magnetogram:
+mhs_solve_boundary (2D V-cycles) -> mhs_solve_interior to the config's tolerance (3D V-cycles) ->
+mhs_fields (B, p, rho).  Workload: BASELINE.json configs[2] (257^3 fp64, the configuration the metric
+is quoted on).  `value` = 3D V-cycles done by all ranks in the K timed steps / device time of those
+steps (so the 2D solve and the field recovery are inside the denominator); inputs are resident in HBM.
+`e2e` = the same through the *_host entry points of the C ABI: pinned-host Bz0 in, pinned-host
+B, p, rho out, copies inside the timed region.  N > 1: one process per GPU, independent magnetograms
+per rank ("replicas only", no data-path collective), max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on this box's host cores on a bounded
+sample of the same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "V-cycles/s (3D, whole path: boundary solve + interior solve to tol + fields) at 257^3 fp64"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def oracle_sample(w, cycles):
+    """The oracle as it stands on a bounded sample: the 2D boundary solve (cheap) to set up, then
+    `cycles` 3D V-cycles at full size, timed.  Returns (V-cycles/s, seconds, threads)."""
+    import numpy as np
+    import oracle
+    P0, _ = oracle.solve_boundary(w.Bz0, (w.Lx, w.Ly), omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=w.tol)
+    P = np.zeros(w.shape); P[0] = P0
+    c = 1.0 + w.f
+    t0 = time.perf_counter()
+    for _ in range(cycles):
+        P = oracle.vcycle3(P, None, c, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+    dt = time.perf_counter() - t0
+    return cycles / dt, dt, oracle.num_threads()
+
+
+def run_reference(args, w, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    per_step = 1 if w.npoints > 5e7 else 2
+    for _ in range(args.warmup and 1):
+        oracle_sample(w, 1)
+    tot_c, tot_t, thr = 0, 0.0, 1
+    for _ in range(args.steps):
+        v, dt, thr = oracle_sample(w, per_step)
+        tot_c += per_step; tot_t += dt
+    val = tot_c / tot_t
+    sample = "%d V-cycles of the 3D interior solve per step at full size (%dx%dx%d), 2D solve and fields untimed" % (
+        per_step, w.nx, w.ny, w.nz)
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "V-cycles/s", "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+           "cpu_baseline": {"value": val, "unit": "V-cycles/s", "cores": thr, "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": "V-cycles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2 = 257^3 fp64)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flags", type=int, default=0, help="mhs_options.flags (1 = reference kernels)")
+    args = ap.parse_args()
+
+    from paper_1307_6720_b200 import inputs
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    w = inputs.config(args.config, replica=rank)
+    cfg = {"workload": "BASELINE.json configs[%d]: %dx%dx%d %s, f(z)=%g*exp(-%g z), alpha=%g, V(%d,%d), omega=2/3, tol %g; "
+                       "one seeded magnetogram per rank" % (args.config, w.nx, w.ny, w.nz, w.dtype, w.a, w.kappa, w.alpha,
+                                                            w.n_pre, w.n_post, w.tol),
+           "grid": [w.nx, w.ny, w.nz], "parallelism": "replicas x%d (no collective on the data path)" % world,
+           "l2": "no flush: per-step working set (2 x %.0f MB iterate buffers + 5 x %.0f MB outputs) exceeds the 126 MB L2"
+                 % (w.npoints * 8 / 1e6, w.npoints * 8 / 1e6)}
+    if args.impl == "reference":
+        return run_reference(args, w, cfg)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1307_6720_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl ours needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dt = torch.float64 if w.dtype == "f64" else torch.float32
+    es = 8 if w.dtype == "f64" else 4
+    N = w.npoints
+    S = binding.Solver.from_workload(w, profile=1, flags=args.flags)
+    bz_dev = torch.as_tensor(w.Bz0, dtype=dt, device="cuda").contiguous()
+    bz_host = torch.as_tensor(w.Bz0, dtype=dt).contiguous().pin_memory()
+    Bd = torch.empty(3 * N, dtype=dt, device="cuda"); pd = torch.empty(N, dtype=dt, device="cuda"); rd = torch.empty(N, dtype=dt, device="cuda")
+    Bh = torch.empty(3 * N, dtype=dt).pin_memory(); ph = torch.empty(N, dtype=dt).pin_memory(); rh = torch.empty(N, dtype=dt).pin_memory()
+
+    def step(host):
+        ib = S.solve_boundary(bz_host if host else bz_dev)
+        ii = S.solve_interior(w.tol, w.max_cycles)
+        if host:
+            S.fields(Bh, ph, rh, host=True)
+        else:
+            S.fields(Bd, pd, rd)
+        return ib["cycles"], ii["cycles"], ii
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(host, steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        c2 = c3 = 0
+        last = None
+        for _ in range(steps):
+            a, b, last = step(host)
+            c2 += a; c3 += b
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+            cc = torch.tensor([c3], device="cuda", dtype=torch.float64)
+            dist.all_reduce(cc, op=dist.ReduceOp.SUM)
+            c3_all = int(cc.item())
+        else:
+            c3_all = c3
+        return ms, c2, c3, c3_all, last
+
+    for _ in range(max(args.warmup, 0)):
+        step(False)
+    step(True)  # warm the host path (staging buffer allocation) outside the timed regions
+    S.reset_profile()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ms, c2, c3, c3_all, last = timed(False, args.steps)
+    prof = S.profile()
+    clk = clocks.stop() if rank == 0 else None
+    S.reset_profile()
+    ms_e2e, _, _, c3_all_e2e, _ = timed(True, args.steps)
+
+    # ---- roofline of the dominant kernel: the finest-level smoother ----
+    peak, peak_src = peaks()
+    n_int = (w.nx - 2) * (w.ny - 2) * (w.nz - 2)
+    launches = prof["launches"]["smooth_l0"]
+    sweeps = prof["sweeps_l0"]
+    t_smooth_ms = prof["ms"]["smooth_l0"]
+    # algorithmic bytes: read u + write u' once per launch, whatever the number of sweeps fused in it
+    # (2w/s per update, s sweeps per launch) -> 2*w*n_int per launch
+    bytes_per_launch = 2.0 * es * n_int
+    achieved = bytes_per_launch * launches / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get("smooth_l0_dram_bytes_per_launch_%d" % w.nx)
+        except Exception:
+            traffic = None
+    roof = {"bound": "hbm", "kernel": "finest-level weighted-Jacobi smoother (kernel class smooth_l0)",
+            "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
+            "frac_of_8TBs_nominal": achieved / 8000.0, "traffic": traffic,
+            "launches": launches, "sweeps": sweeps, "sweeps_per_launch": (sweeps / launches) if launches else None,
+            "avg_launch_us": 1e3 * t_smooth_ms / launches if launches else None,
+            "algorithmic_bytes_per_launch": bytes_per_launch,
+            "smoother_gpts_per_s": n_int * sweeps / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0,
+            "smoother_share_of_step": t_smooth_ms / ms}
+
+    out = {"metric": METRIC, "value": c3_all / (ms * 1e-3), "unit": "V-cycles/s", "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": w.dtype, "data": "synthetic", "config": cfg,
+           "cycles_per_step": {"boundary_2d": c2 / args.steps, "interior_3d": c3 / args.steps},
+           "converged": bool(last["converged"]), "r_final_over_r0": last["r_final"] / last["r0"] if last["r0"] else 0.0,
+           "clocks": clk, "roofline": roof,
+           "e2e": {"value": c3_all_e2e / (ms_e2e * 1e-3), "unit": "V-cycles/s", "ms_per_step": ms_e2e / args.steps,
+                   "h2d_bytes_per_step": w.nx * w.ny * es, "d2h_bytes_per_step": 5 * N * es},
+           "gpu_launches": prof["total_launches"],
+           "kernel_launches_by_class": prof["launches"]}
+    S.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, dtm, thr = oracle_sample(w, 2 if N < 5e7 else 1)
+        out["cpu_baseline"] = {"value": v, "unit": "V-cycles/s", "cores": thr, "kind": "oracle",
+                               "sample": "%d V-cycles of the 3D interior solve at %dx%dx%d (%.1f s); 2D solve and fields not timed"
+                                         % (2 if N < 5e7 else 1, w.nx, w.ny, w.nz, dtm)}
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -140,10 +140,11 @@ _SPECS = {
 }
 
 
-def config(index: int, shrink: int = 1) -> Workload:
+def config(index: int, shrink: int = 1, replica: int = 0) -> Workload:
     """BASELINE.json `configs[index]`.  `shrink` = 2^s divides the number of intervals per axis
     (same domain, same sources) -- used by parity tests that need an oracle-sized version of
-    the big configs; shrink=1 is the configuration itself."""
+    the big configs; shrink=1 is the configuration itself.  `replica` r > 0 draws an independent
+    magnetogram of the same recipe (seed + 1000003 r): one per rank in multi-GPU replica runs."""
     s = _SPECS[index]
     nx, ny, nz = [(m - 1) // shrink + 1 for m in s["n"]]
     Lx, Ly, Lz = s["L"]
@@ -155,7 +156,7 @@ def config(index: int, shrink: int = 1) -> Workload:
         # one bipole, deterministic (BASELINE configs[0]); no flux zeroing needed (C18/C19)
         w.Bz0 = gaussian_patches(nx, ny, Lx, Ly, [1.0, -1.0], [0.1, 0.1], [0.4, 0.6], [0.5, 0.5])
     else:
-        rng = SplitMix64(SEED_BASE + index)
+        rng = SplitMix64(SEED_BASE + index + 1000003 * replica)
         bz = random_patches(rng, s["patches"], nx, ny, Lx, Ly, *s["sig"])
         if "noise" in s:
             bz = bz + s["noise"] * rng.uniform(-1.0, 1.0, nx * ny).reshape(ny, nx)
