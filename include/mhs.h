@@ -170,7 +170,9 @@ mhs_status mhs_op_smooth(mhs_ctx *ctx, int dim, int level, int sweeps);   /* u <
 mhs_status mhs_op_residual(mhs_ctx *ctx, int dim, int level);             /* r <- rhs - L u           */
 mhs_status mhs_op_restrict(mhs_ctx *ctx, int dim, int level);             /* rhs_{l+1} <- R (rhs - L u)_l */
 mhs_status mhs_op_prolong(mhs_ctx *ctx, int dim, int level);              /* u_l <- u_l + P u_{l+1}   */
-mhs_status mhs_op_vcycle(mhs_ctx *ctx, int dim, int level);               /* one V-cycle from `level` */
+mhs_status mhs_op_vcycle(mhs_ctx *ctx, int dim, int level);               /* one V-cycle from `level`: level 0
+                                                                             continues from u, levels >= 1 start
+                                                                             from u = 0 as inside a cycle      */
 mhs_status mhs_op_resnorm(mhs_ctx *ctx, int dim, int level, double *out_host); /* ||rhs - L u||_2     */
 
 #ifdef __cplusplus

@@ -239,55 +239,116 @@ int kc_for(const Level& lv, int l, int what /*0 smooth 1 restrict 2 prolong 3 no
     return what;
 }
 
-void smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const int* done)
+bool use_fast(const mhs_ctx* ctx, const Level& lv)
+{
+    return !(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fast_ok(ctx, lv);
+}
+
+int tail_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->tail3 : ctx->tail2; }
+
+// `sweeps` Jacobi sweeps on level l, ping-ponging lv.u <-> lv.tmp.  want_norm: the first sweep also leaves
+// the partial sums of ||rhs - L u||^2 of ITS INPUT in ctx->partial (returned count; 0 = not computed).
+long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const int* done, bool want_norm = false)
 {
     Level& lv = Ls[l];
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    const bool fast = use_fast(ctx, lv);
+    long long npart = 0;
     for (int s = 0; s < sweeps; ++s) {
         Scope sc(ctx, kc_for(lv, l, 0));
-        launch_smooth_ref(ctx, lv, lv.u, rhs, lv.tmp, done);
+        if (fast) {
+            const long long n = launch_smooth_z(ctx, lv, lv.u, rhs, lv.tmp, (want_norm && s == 0) ? 1 : 0, ctx->dir, done);
+            if (want_norm && s == 0) npart = n;
+            ctx->dir ^= 1;
+        } else {
+            launch_smooth_ref(ctx, lv, lv.u, rhs, lv.tmp, done);
+        }
         std::swap(lv.u, lv.tmp);
         if (lv.dim == 3 && l == 0) ctx->prof.sweeps_l0 += 1;
     }
+    return npart;
 }
 
-void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done)
+// Partial sums of ||rhs - L u||^2 on level l -> ctx->partial; returns their count.
+long long resnorm_partials(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done)
 {
     Level& lv = Ls[l];
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    Scope sc(ctx, kc_for(lv, l, 3));
+    if (use_fast(ctx, lv)) return launch_smooth_z(ctx, lv, lv.u, rhs, nullptr, 2, 0, done);
+    return launch_resnorm_partial_ref(ctx, lv, lv.u, rhs, done);
+}
+
+void norm_final(mhs_ctx* ctx, const Level& lv, int l, long long n, int mode)
+{
+    Scope sc(ctx, kc_for(lv, l, 3));
+    launch_norm_final(ctx, n, mode);
+}
+
+// One V-cycle from level l (SURVEY 8(c) "V(u,rhs,l)").  Levels >= 1 start from u = 0.  At l == 0 with
+// fuse_norm the norm of the incoming iterate's residual is taken inside the first pre-sweep and the
+// stop rule (norm_final mode 1) is evaluated right after it, before the rest of the cycle is allowed to run.
+void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool fuse_norm = false)
+{
+    Level& lv = Ls[l];
+    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    if (l > 0 && l >= tail_of(ctx, Ls)) {
+        Scope sc(ctx, kc_for(lv, l, 0));
+        launch_tail(ctx, Ls, l, done);
+        return;
+    }
     if (lv.coarsest) {
         Scope sc(ctx, kc_for(lv, l, 0));
         launch_coarse_solve(ctx, lv, lv.u, rhs, done);
         return;
     }
     Level& co = Ls[l + 1];
-    smooth(ctx, Ls, l, ctx->opt.n_pre, done);
+    const bool fast = use_fast(ctx, lv);
+    int n_pre = ctx->opt.n_pre;
+    if (l > 0) {  // zero initial guess
+        Scope sc(ctx, kc_for(lv, l, 0));
+        if (fast && n_pre >= 1) {
+            launch_scale_rhs(ctx, lv, rhs, lv.u, done);  // first sweep from zero: u = (omega/D) rhs
+            n_pre -= 1;
+        } else {
+            cudaMemsetAsync(field_base(ctx, lv, lv.u), 0, (size_t)lv.alloc * ctx->es, ctx->stream);
+        }
+    }
+    if (fuse_norm && l == 0) {
+        const long long np = smooth(ctx, Ls, l, 1, nullptr, true);  // must run even when `done` is about to be raised
+        norm_final(ctx, lv, l, np, 1);
+        smooth(ctx, Ls, l, n_pre - 1, done);
+    } else {
+        smooth(ctx, Ls, l, n_pre, done);
+    }
     {
         Scope sc(ctx, kc_for(lv, l, 1));
-        launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, done);
-        launch_restrict_ref(ctx, lv, lv.r, co, co.rhs, done);
-        if (!co.coarsest) cudaMemsetAsync(field_base(ctx, co, co.u), 0, (size_t)co.alloc * ctx->es, ctx->stream);
+        if (fast) {
+            launch_resid_restrict_z(ctx, lv, lv.u, rhs, co, co.rhs, ctx->dir, done);
+            ctx->dir ^= 1;
+        } else {
+            launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, done);
+            launch_restrict_ref(ctx, lv, lv.r, co, co.rhs, done);
+        }
     }
     vcycle(ctx, Ls, l + 1, done);
     {
         Scope sc(ctx, kc_for(lv, l, 2));
-        launch_prolong_ref(ctx, lv, lv.u, co, co.u, done);
+        if (fast) {
+            launch_prolong_v(ctx, lv, lv.u, co, co.u, ctx->dir, done);
+            ctx->dir ^= 1;
+        } else {
+            launch_prolong_ref(ctx, lv, lv.u, co, co.u, done);
+        }
     }
     smooth(ctx, Ls, l, ctx->opt.n_post, done);
 }
 
-void resnorm(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int mode, const int* done)
-{
-    Level& lv = Ls[l];
-    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
-    Scope sc(ctx, kc_for(lv, l, 3));
-    const long long n = launch_resnorm_partial_ref(ctx, lv, lv.u, rhs, done);
-    launch_norm_final(ctx, n, mode);
-}
-
-// Solve loop shared by the 2D and 3D drivers: cycles run speculatively in chunks behind the
-// device-side stop flag; the host reads the control block once per chunk (C10 stop rule is exact:
-// every kernel of a cycle issued after the flag was raised returns without touching anything).
+// Solve loop shared by the 2D and 3D drivers.  Unit q = [norm of iterate q-1 -> stop rule] + [V-cycle q];
+// units run speculatively in chunks behind the device-side stop flag and the host reads the control block
+// once per chunk.  The stop rule (C10) is exact: once the flag is up every later kernel returns at once, and
+// the only kernel that may already have run -- the first pre-sweep, which carries the norm -- writes the
+// ping-pong buffer, never the iterate.  iter_buf[q] remembers which buffer holds iterate q.
 mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_cycles, double r0_known,
                       mhs_solve_info* info)
 {
@@ -299,25 +360,54 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
     h->r0 = r0_known;
     h->stag_on = ctx->es == 4;
     CK(cudaMemcpyAsync(ctx->ctl, h, sizeof(Ctl), cudaMemcpyHostToDevice, ctx->stream));
-    if (!(r0_known > 0.0)) resnorm(ctx, Ls, 0, 0, nullptr);
-    // The ping-pong buffers of the finest level swap roles once per sweep; with an odd number of
-    // sweeps per cycle a skipped (speculative) cycle would leave them swapped, so sync every cycle.
-    const bool odd = ((ctx->opt.n_pre + ctx->opt.n_post) & 1) != 0;
-    const int chunk = ((ctx->opt.flags & MHS_FLAG_SYNC_EACH_CYCLE) || odd) ? 1 : 4;
+    Level& l0 = Ls[0];
+    const int* done = &ctx->ctl->done;
+    const bool fuse = use_fast(ctx, l0) && ctx->opt.n_pre >= 1 && !l0.coarsest;
+    const bool sync_each = (ctx->opt.flags & MHS_FLAG_SYNC_EACH_CYCLE) != 0;
+    std::vector<void*> iter_buf(1, l0.u);
     int issued = 0;
+    bool trailing = false;
     while (true) {
-        const int n = std::min(chunk, max_cycles - issued);
+        // How many units to issue before the next read-back: 4 to start with, then the number the observed
+        // convergence factor predicts are still needed (+1: a cycle's norm is taken by the unit after it),
+        // so that hardly any speculative unit is wasted.  Purely a scheduling choice: results do not depend on it.
+        int want = 4;
+        if (h->cycles >= 2 && h->cycles <= MHS_HISTORY_LEN) {
+            const double rl = h->hist[h->cycles - 1], rp = h->hist[h->cycles - 2];
+            const double target = tol * h->r0;
+            if (rl > 0.0 && rp > rl && target > 0.0 && rl > target) {
+                const double need = std::ceil(std::log(target / rl) / std::log(rl / rp));
+                want = (int)std::min(8.0, std::max(1.0, h->cycles + need + 1 - issued));
+            }
+        }
+        const int n = std::min(sync_each ? 1 : want, max_cycles - issued);
         for (int q = 0; q < n; ++q) {
-            vcycle(ctx, Ls, 0, &ctx->ctl->done);
-            resnorm(ctx, Ls, 0, 1, &ctx->ctl->done);
+            if (fuse) {
+                vcycle(ctx, Ls, 0, done, true);
+            } else {
+                const long long np = resnorm_partials(ctx, Ls, 0, done);
+                norm_final(ctx, l0, 0, np, 1);
+                vcycle(ctx, Ls, 0, done);
+            }
+            iter_buf.push_back(l0.u);
         }
         issued += n;
+        if (issued >= max_cycles) {  // norm of the last iterate
+            const long long np = resnorm_partials(ctx, Ls, 0, done);
+            norm_final(ctx, l0, 0, np, 1);
+            trailing = true;
+        }
         CK(cudaMemcpyAsync(h, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
         CK(cudaStreamSynchronize(ctx->stream));
-        if (h->done || issued >= max_cycles) break;
+        if (h->done || trailing) break;
     }
     drain_events(ctx);
     CK(cudaGetLastError());
+    // put the final iterate back under the name `u`
+    if (l0.tmp && h->cycles >= 0 && h->cycles < (int)iter_buf.size()) {
+        void* fin = iter_buf[h->cycles];
+        if (fin != l0.u) std::swap(l0.u, l0.tmp);
+    }
     if (info) {
         info->cycles = h->cycles;
         info->r0 = h->r0;
@@ -455,7 +545,18 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ft[3 * nz + k] = ctx->rho_b[k];
     }
     if ((st = upload(ctx, &ctx->prof_tab, ft))) return st;
+    {
+        int dev = 0;
+        cudaDeviceProp pr;
+        CK(cudaGetDevice(&dev));
+        CK(cudaGetDeviceProperties(&pr, dev));
+        ctx->num_sms = pr.multiProcessorCount;
+    }
+    const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
+    ctx->tail3 = ref ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
+    ctx->tail2 = ref ? (int)ctx->L2.size() : tail_start(ctx, ctx->L2, 216 * 1024);
     ctx->npartial = std::max(resnorm_partial_capacity(ctx->L3[0]), resnorm_partial_capacity(ctx->L2[0]));
+    for (const Level& lv : ctx->L3) ctx->npartial = std::max(ctx->npartial, smooth_z_partial_capacity(ctx, lv));
     CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
     CK(cudaMalloc((void**)&ctx->ctl, sizeof(Ctl)));
     CK(cudaMemset(ctx->ctl, 0, sizeof(Ctl)));
@@ -716,8 +817,13 @@ mhs_status mhs_op_restrict(mhs_ctx* ctx, int dim, int level)
     Level& lv = (*Ls)[level];
     if (lv.coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "no level below the coarsest");
     Scope sc(ctx, kc_for(lv, level, 1));
-    launch_residual_ref(ctx, lv, lv.u, (dim == 3 && level == 0) ? nullptr : lv.rhs, lv.r, nullptr);
-    launch_restrict_ref(ctx, lv, lv.r, (*Ls)[level + 1], (*Ls)[level + 1].rhs, nullptr);
+    const void* rhs = (dim == 3 && level == 0) ? nullptr : lv.rhs;
+    if (use_fast(ctx, lv)) {
+        launch_resid_restrict_z(ctx, lv, lv.u, rhs, (*Ls)[level + 1], (*Ls)[level + 1].rhs, 0, nullptr);
+    } else {
+        launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, nullptr);
+        launch_restrict_ref(ctx, lv, lv.r, (*Ls)[level + 1], (*Ls)[level + 1].rhs, nullptr);
+    }
     CK(cudaGetLastError());
     return MHS_OK;
 }
@@ -731,7 +837,8 @@ mhs_status mhs_op_prolong(mhs_ctx* ctx, int dim, int level)
     Level& lv = (*Ls)[level];
     if (lv.coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "no level below the coarsest");
     Scope sc(ctx, kc_for(lv, level, 2));
-    launch_prolong_ref(ctx, lv, lv.u, (*Ls)[level + 1], (*Ls)[level + 1].u, nullptr);
+    if (use_fast(ctx, lv)) launch_prolong_v(ctx, lv, lv.u, (*Ls)[level + 1], (*Ls)[level + 1].u, 0, nullptr);
+    else launch_prolong_ref(ctx, lv, lv.u, (*Ls)[level + 1], (*Ls)[level + 1].u, nullptr);
     CK(cudaGetLastError());
     return MHS_OK;
 }
@@ -753,7 +860,10 @@ mhs_status mhs_op_resnorm(mhs_ctx* ctx, int dim, int level, double* out_host)
     std::vector<Level>* Ls;
     mhs_status st = check_level(ctx, dim, level, &Ls);
     if (st) return st;
-    resnorm(ctx, *Ls, level, 2, nullptr);
+    {
+        const long long np = resnorm_partials(ctx, *Ls, level, nullptr);
+        norm_final(ctx, (*Ls)[level], level, np, 2);
+    }
     CK(cudaMemcpyAsync(ctx->ctl_host, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     drain_events(ctx);

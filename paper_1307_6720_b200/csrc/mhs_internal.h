@@ -33,7 +33,8 @@ struct Ctl {  // device-side solve control block (one per context)
     int cycles;      // cycles completed in this call
     int max_cycles;
     int nan_seen;
-    int stag_on, stag_count, stagnated, pad_;  // fp32 stagnation rule (C20)
+    int stag_on, stag_count, stagnated;
+    int units;       // cycles completed so far (device-side counter of the unit scheme)  // fp32 stagnation rule (C20)
     double r0, tol, r_last;
     double hist[MHS_HISTORY_LEN];
 };
@@ -76,6 +77,9 @@ struct mhs_ctx {
     double r0_interior = 0;
     mhs_profile prof{};
     int cur_kc = MHS_KC_PACK;  // kernel class the launchers charge
+    int num_sms = 148;
+    int tail3 = 1 << 30, tail2 = 1 << 30;  // first level handled by the single-CTA tail kernel
+    int dir = 0;               // z traversal direction of the next big kernel (alternates)
     std::vector<mhs::Ev> ev_pending;
     std::vector<cudaEvent_t> ev_pool;
     std::string err;
@@ -100,5 +104,16 @@ void launch_norm_final(mhs_ctx* c, long long n, int mode);
 void launch_pack(mhs_ctx* c, const Level& lv, const void* dense, void* dst, bool keep_bottom, bool negate);
 void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense);
 void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
+
+// ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
+bool fast_ok(const mhs_ctx* c, const Level& lv);
+// mode 0: sweep; 1: sweep + partial sums of the INPUT's ||rhs - L u||^2; 2: partial sums only.  Returns #partials.
+long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done);
+long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
+void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);
+void launch_resid_restrict_z(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
+void launch_prolong_v(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, int reverse, const int* done);
+int tail_start(const mhs_ctx* c, const std::vector<Level>& Ls, size_t budget_bytes);
+void launch_tail(mhs_ctx* c, std::vector<Level>& Ls, int l0, const int* done);
 
 }  // namespace mhs

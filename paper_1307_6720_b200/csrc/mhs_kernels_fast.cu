@@ -1,0 +1,429 @@
+// Tuned 3D kernels of libmhs_b200 for sm_100a (HBM-bound 7-point stencils; no tensor cores: nothing
+// here is a dense contraction).  Common scheme ("flat z-streaming"):
+//
+//   * The aliased Dirichlet layout (mhs_internal.h) makes every plane one FLAT array: the x-neighbours
+//     of an element are flat-1 / flat+1 even across row ends (what sits there is a wall zero), the
+//     y-neighbours are flat-+sx.  A thread owns R vertically adjacent 128-bit vectors (double2 / float4)
+//     and walks up in z keeping the planes k-1, k, k+1 of its R vectors in registers, so each element of
+//     the iterate is loaded once per kernel by its owner (+ the two halo rows of the R-row strip, which
+//     hit L1/L2) and z-neighbours never touch memory.
+//   * x-neighbours across vectors come from warp shuffles; only lanes 0 and 31 issue a scalar load.
+//   * c_k/hx^2, c_k/hy^2, omega/D_k are per-plane scalars from a small table (L1-resident).
+//   * The residual rhs - L u of the INPUT iterate is an intermediate of the Jacobi update, so its squared
+//     norm is accumulated for free (warp shuffles + one partial per block): the stop test needs no pass of
+//     its own.
+//   * Grids are sized to fill a whole number of waves on the 148 SMs (z-chunk length is the free parameter);
+//     consecutive kernels traverse the z-chunks in opposite order so that the tail of what the previous
+//     kernel wrote is still in the 126 MB L2 when the next one starts.
+#include "mhs_device.cuh"
+
+namespace mhs {
+
+template <typename T> struct VN;
+template <> struct VN<double> { static constexpr int N = 2; };
+template <> struct VN<float> { static constexpr int N = 4; };
+
+template <typename T>
+struct __align__(16) Vec {
+    T v[VN<T>::N];
+};
+
+template <typename T>
+__device__ __forceinline__ Vec<T> ldv(const T* p) { return *reinterpret_cast<const Vec<T>*>(p); }
+template <typename T>
+__device__ __forceinline__ void stv(T* p, const Vec<T>& a) { *reinterpret_cast<Vec<T>*>(p) = a; }
+
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ float shfl_up1(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ float shfl_dn1(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// rhs - L u for the V elements of one vector.  cw/ce: the elements left / right of the vector.
+template <typename T>
+__device__ __forceinline__ void residual_vec(const Vec<T>& c, T cw, T ce, const Vec<T>& n, const Vec<T>& s, const Vec<T>& up,
+                                             const Vec<T>& dn, const Vec<T>* f, T cx, T cy, T cz, T a2, Vec<T>& r)
+{
+    constexpr int V = VN<T>::N;
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+        const T w = e == 0 ? cw : c.v[e - 1];
+        const T ea = e == V - 1 ? ce : c.v[e + 1];
+        T lu = cx * lap1<T>(ea, w, c.v[e]) + cy * lap1<T>(n.v[e], s.v[e], c.v[e]);
+        lu += cz * lap1<T>(up.v[e], dn.v[e], c.v[e]) + a2 * c.v[e];
+        r.v[e] = (f ? f->v[e] : T(0)) - lu;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// One weighted-Jacobi sweep (a2) over the z-chunk of this block.
+//   STORE : write out = u + (omega/D_k) r          NORM : accumulate sum r^2 into partial[block]
+// Work item q <-> (row group g, x vector xv): rows j0 = g*R .. j0+R-1, elements i0 = xv*V .. i0+V-1.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM>
+__global__ void __launch_bounds__(128) k_smooth_z(LP<T> p, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ out,
+                                                   int kchunk, int nzc, int reverse, double* __restrict__ partial,
+                                                   const int* __restrict__ done)
+{
+    if (done && *done) return;
+    constexpr int V = VN<T>::N;
+    const int nvx = p.sx / V;
+    const int ngroups = (p.sy + R - 1) / R;
+    const long long total = (long long)ngroups * nvx;
+    const long long q0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool active = q0 < total;
+    const long long q = active ? q0 : 0;   // idle lanes shadow item 0: its first element is a wall zero, which
+                                           // is exactly the right-hand neighbour the last active lane needs
+    const int g = (int)(q / nvx), xv = (int)(q - (long long)g * nvx);
+    const int i0 = xv * V, j0 = g * R;
+    const int lane = threadIdx.x & 31;
+    const int zc = reverse ? nzc - 1 - (int)blockIdx.y : (int)blockIdx.y;
+    const int kb = 1 + zc * kchunk;
+    const int ke = min(kb + kchunk, p.nz - 1);
+    const long long base = i0 + (long long)p.sx * j0;
+    const T* tab = p.tab;
+
+    Vec<T> cm[R], cc[R], cp[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        cm[r] = ldv(u + base + (long long)p.sx * r + p.sp * (kb - 1));
+        cc[r] = ldv(u + base + (long long)p.sx * r + p.sp * kb);
+    }
+    double acc = 0.0;
+    for (int k = kb; k < ke; ++k) {
+        const T* pl = u + base + p.sp * k;
+#pragma unroll
+        for (int r = 0; r < R; ++r) cp[r] = ldv(pl + p.sp + (long long)p.sx * r);
+        const Vec<T> ntop = ldv(pl + (long long)p.sx * R);
+        const Vec<T> sbot = ldv(pl - p.sx);
+        const T cx = tab[k], cy = tab[p.nz + k], wk = tab[3 * p.nz + k];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            T cw = shfl_up1(cc[r].v[V - 1]);
+            T ce = shfl_dn1(cc[r].v[0]);
+            if (lane == 0) cw = pl[(long long)p.sx * r - 1];
+            if (lane == 31) ce = pl[(long long)p.sx * r + V];
+            Vec<T> f, res;
+            if (HAS_RHS) f = ldv(rhs + base + p.sp * k + (long long)p.sx * r);
+            residual_vec<T>(cc[r], cw, ce, r == R - 1 ? ntop : cc[r + 1 < R ? r + 1 : r], r == 0 ? sbot : cc[r > 0 ? r - 1 : 0],
+                            cp[r], cm[r], HAS_RHS ? &f : nullptr, cx, cy, p.cz, p.a2, res);
+            const bool rowok = active && (j0 + r < p.sy) && (j0 + r > 0);
+            Vec<T> o;
+#pragma unroll
+            for (int e = 0; e < V; ++e) {
+                const bool wall = (i0 + e == 0);
+                o.v[e] = wall ? cc[r].v[e] : cc[r].v[e] + wk * res.v[e];
+                if (NORM && rowok && !wall) acc += (double)res.v[e] * (double)res.v[e];
+            }
+            if (STORE && rowok) stv(out + base + p.sp * k + (long long)p.sx * r, o);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) { cm[r] = cc[r]; cc[r] = cp[r]; }
+    }
+    if (NORM) {
+        acc = block_sum<128>(acc);
+        if (threadIdx.x == 0) partial[blockIdx.x + (long long)gridDim.x * blockIdx.y] = acc;
+    }
+}
+
+// u = (omega/D_k) rhs : the first sweep from the zero initial guess of a coarse-grid correction
+// (u + w (rhs - L 0) with u = 0), saving the zero fill and one read of u.
+template <typename T>
+__global__ void __launch_bounds__(256) k_scale_rhs(LP<T> p, const T* __restrict__ rhs, T* __restrict__ u, const int* __restrict__ done)
+{
+    if (done && *done) return;
+    constexpr int V = VN<T>::N;
+    const long long nv = p.sp / V;
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = blockIdx.y + 1;
+    if (q >= nv) return;
+    const T wk = p.tab[3 * p.nz + k];
+    Vec<T> f = ldv(rhs + q * V + p.sp * k);
+#pragma unroll
+    for (int e = 0; e < V; ++e) f.v[e] *= wk;
+    stv(u + q * V + p.sp * k, f);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Residual + full-weighting restriction fused (a3 + a4): rhs_c = R (rhs - L u), never storing r.
+// A thread owns rows j0-1 .. j0+R-1 (R even, j0 even) of one x vector: the residuals of R+1 rows give the
+// R/2 coarse rows j0/2 .. ; the x part of the weighting takes the odd left neighbour from the lane below
+// (warps overlap by one vector: lane 0 only feeds lane 1), the z part is accumulated while streaming:
+// odd fine planes close one coarse plane with weight 1/4 and open the next.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int R, bool HAS_RHS>
+__global__ void __launch_bounds__(128) k_resid_restrict_z(LP<T> p, const T* __restrict__ u, const T* __restrict__ rhs, int csx,
+                                                           long long csp, int cnz, T* __restrict__ rc, int Kchunk, int nzc, int reverse,
+                                                           const int* __restrict__ done)
+{
+    if (done && *done) return;
+    constexpr int V = VN<T>::N;
+    constexpr int VC = V / 2;
+    constexpr int RR = R + 1;
+    const int nvx = p.sx / V;
+    const int ngroups = (p.sy + R - 1) / R;
+    const long long total = (long long)ngroups * nvx;
+    const int lane = threadIdx.x & 31;
+    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long q0 = warp * 31 + lane - 1;
+    const bool active = q0 >= 0 && q0 < total && lane > 0;
+    const long long q = (q0 >= 0 && q0 < total) ? q0 : 0;
+    const int g = (int)(q / nvx), xv = (int)(q - (long long)g * nvx);
+    const int i0 = xv * V, j0 = g * R;
+    const int zc = reverse ? nzc - 1 - (int)blockIdx.y : (int)blockIdx.y;
+    const int Kb = 1 + zc * Kchunk;
+    const int Ke = min(Kb + Kchunk, cnz - 1);
+    if (Kb >= Ke) return;
+    const long long base = i0 + (long long)p.sx * (j0 - 1);   // row t = 0 is fine row j0-1
+    const T* tab = p.tab;
+
+    Vec<T> cm[RR], cc[RR], cp[RR];
+    const int k0 = 2 * Kb - 1;
+#pragma unroll
+    for (int t = 0; t < RR; ++t) {
+        cm[t] = ldv(u + base + (long long)p.sx * t + p.sp * (k0 - 1));
+        cc[t] = ldv(u + base + (long long)p.sx * t + p.sp * k0);
+    }
+    T accA[R / 2][VC];
+#pragma unroll
+    for (int s = 0; s < R / 2; ++s)
+#pragma unroll
+        for (int m = 0; m < VC; ++m) accA[s][m] = T(0);
+
+    for (int k = k0; k <= 2 * Ke - 1; ++k) {
+        const T* pl = u + base + p.sp * k;
+#pragma unroll
+        for (int t = 0; t < RR; ++t) cp[t] = ldv(pl + p.sp + (long long)p.sx * t);
+        const Vec<T> ntop = ldv(pl + (long long)p.sx * RR);
+        const Vec<T> sbot = ldv(pl - p.sx);
+        const T cx = tab[k], cy = tab[p.nz + k];
+        T tx[RR][VC];
+#pragma unroll
+        for (int t = 0; t < RR; ++t) {
+            T cw = shfl_up1(cc[t].v[V - 1]);
+            T ce = shfl_dn1(cc[t].v[0]);
+            if (lane == 0) cw = pl[(long long)p.sx * t - 1];
+            if (lane == 31) ce = pl[(long long)p.sx * t + V];
+            Vec<T> f, res;
+            if (HAS_RHS) f = ldv(rhs + base + p.sp * k + (long long)p.sx * t);
+            residual_vec<T>(cc[t], cw, ce, t == RR - 1 ? ntop : cc[t + 1 < RR ? t + 1 : t], t == 0 ? sbot : cc[t > 0 ? t - 1 : 0],
+                            cp[t], cm[t], HAS_RHS ? &f : nullptr, cx, cy, p.cz, p.a2, res);
+            const int j = j0 - 1 + t;
+            const bool rowok = j > 0 && j < p.sy;   // wall rows (and the aliased rows beyond them) carry r = 0
+#pragma unroll
+            for (int e = 0; e < V; ++e)
+                if (!rowok || (i0 + e == 0)) res.v[e] = T(0);
+            // x weighting: coarse element m sits on fine element 2m of this vector
+            const T left = shfl_up1(res.v[V - 1]);
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                const T l = m == 0 ? left : res.v[2 * m - 1];
+                tx[t][m] = T(0.5) * res.v[2 * m] + T(0.25) * (l + res.v[2 * m + 1]);
+            }
+        }
+        const bool odd = (k & 1) != 0;
+#pragma unroll
+        for (int s = 0; s < R / 2; ++s) {
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                const T ty = T(0.5) * tx[2 * s + 1][m] + T(0.25) * (tx[2 * s][m] + tx[2 * s + 2][m]);
+                if (!odd) {
+                    accA[s][m] += T(0.5) * ty;
+                } else {
+                    const T closed = accA[s][m] + T(0.25) * ty;
+                    accA[s][m] = T(0.25) * ty;
+                    if (k > k0) {
+                        const int K = (k - 1) >> 1;
+                        const int I = (i0 >> 1) + m, J = (j0 >> 1) + s;
+                        if (active && I > 0 && J > 0 && (j0 + 2 * s) < p.sy)
+                            rc[I + (long long)csx * J + csp * K] = closed;
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < RR; ++t) { cm[t] = cc[t]; cc[t] = cp[t]; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Trilinear prolongation + correction (a6): u += P e_c, one fine vector per thread.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) k_prolong_v(int sx, int sy, long long sp, T* __restrict__ u, int csx, long long csp,
+                                                    const T* __restrict__ ec, int reverse, int nzi, const int* __restrict__ done)
+{
+    if (done && *done) return;
+    constexpr int V = VN<T>::N;
+    constexpr int VC = V / 2;
+    const long long nv = sp / V;
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int k = (reverse ? nzi - 1 - (int)blockIdx.y : (int)blockIdx.y) + 1;
+    if (q >= nv) return;
+    const long long flat = q * V;
+    const int j = (int)(flat / sx), i0 = (int)(flat - (long long)j * sx);
+    if (j == 0) return;
+    const int I0 = i0 >> 1, J0 = j >> 1, J1 = (j + 1) >> 1, K0 = k >> 1, K1 = (k + 1) >> 1;
+    // sum the four (J,K) corner rows first, then interpolate in x
+    T c[VC + 1];
+#pragma unroll
+    for (int m = 0; m <= VC; ++m) {
+        const long long o = I0 + m;
+        c[m] = (ec[o + (long long)csx * J0 + csp * K0] + ec[o + (long long)csx * J1 + csp * K0]) +
+               (ec[o + (long long)csx * J0 + csp * K1] + ec[o + (long long)csx * J1 + csp * K1]);
+    }
+    Vec<T> a = ldv(u + flat + sp * k);
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+        const T s = (e & 1) ? (c[e >> 1] + c[(e >> 1) + 1]) : T(2) * c[e >> 1];
+        if (i0 + e != 0) a.v[e] += T(0.125) * s;
+    }
+    stv(u + flat + sp * k, a);
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+static LP<T> lp_of(const mhs_ctx* c, const Level& lv)
+{
+    LP<T> p;
+    p.nx = lv.nx; p.ny = lv.ny; p.nz = lv.nz; p.sx = lv.sx; p.sy = lv.sy; p.sp = lv.sp;
+    p.tab = (const T*)lv.tab;
+    p.cz = (T)(1.0 / (lv.hz * lv.hz));
+    p.a2 = (T)(c->alpha * c->alpha);
+    return p;
+}
+
+bool fast_ok(const mhs_ctx* c, const Level& lv)
+{
+    const int V = c->es == 8 ? 2 : 4;
+    return lv.dim == 3 && !lv.coarsest && lv.sx % V == 0 && lv.sx >= V && lv.nz >= 3;
+}
+
+// z-chunk length such that the grid is (just under) a whole number of waves of `slots` resident blocks.
+static int pick_chunks(long long xy_blocks, int planes, int slots, int min_chunk)
+{
+    int best = 1;
+    double best_score = -1.0;
+    const int maxc = planes / min_chunk > 0 ? planes / min_chunk : 1;
+    for (int nc = 1; nc <= maxc; ++nc) {
+        const int len = (planes + nc - 1) / nc;
+        const int real = (planes + len - 1) / len;
+        const double blocks = (double)xy_blocks * real;
+        const double waves = blocks / slots;
+        const double eff = waves / std::ceil(waves);                  // last-wave quantisation
+        const double halo = (double)len / (len + 2);                  // 2 redundant planes per chunk
+        const double par = std::min(1.0, blocks / slots);             // enough blocks to fill the machine
+        const double score = eff * halo * par;
+        if (score > best_score + 1e-9) { best_score = score; best = real; }
+    }
+    return best;
+}
+
+template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM>
+static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int reverse, const int* done)
+{
+    constexpr int V = VN<T>::N;
+    auto kern = k_smooth_z<T, R, HAS_RHS, STORE, NORM>;
+    static int slots = 0;
+    if (!slots) {
+        int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
+        slots = std::max(1, nb) * c->num_sms;
+    }
+    const long long items = (long long)((lv.sy + R - 1) / R) * (lv.sx / V);
+    const long long xb = (items + 127) / 128;
+    const int planes = lv.nz - 2;
+    const int nzc = pick_chunks(xb, planes, slots, 8);
+    const int kchunk = (planes + nzc - 1) / nzc;
+    const int nzc2 = (planes + kchunk - 1) / kchunk;
+    dim3 grid((unsigned)xb, (unsigned)nzc2);
+    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, lv), (const T*)u, (const T*)rhs, (T*)out, kchunk, nzc2, reverse, c->partial, done);
+    return xb * nzc2;
+}
+
+// mode: 0 = sweep, 1 = sweep + norm of the input residual, 2 = norm only.  Returns the number of partials.
+long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done)
+{
+    count_launch(c);
+#define SZ(T, R)                                                                                              \
+    do {                                                                                                      \
+        if (rhs) {                                                                                            \
+            if (mode == 0) return smooth_z_t<T, R, true, true, false>(c, lv, u, rhs, out, reverse, done);     \
+            if (mode == 1) return smooth_z_t<T, R, true, true, true>(c, lv, u, rhs, out, reverse, done);      \
+            return smooth_z_t<T, R, true, false, true>(c, lv, u, rhs, out, reverse, done);                    \
+        } else {                                                                                              \
+            if (mode == 0) return smooth_z_t<T, R, false, true, false>(c, lv, u, rhs, out, reverse, done);    \
+            if (mode == 1) return smooth_z_t<T, R, false, true, true>(c, lv, u, rhs, out, reverse, done);     \
+            return smooth_z_t<T, R, false, false, true>(c, lv, u, rhs, out, reverse, done);                   \
+        }                                                                                                     \
+    } while (0)
+    if (c->es == 8) SZ(double, 4);
+    else SZ(float, 4);
+#undef SZ
+    return 0;
+}
+
+long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
+{
+    const int V = c->es == 8 ? 2 : 4;
+    const long long items = (long long)((lv.sy + 3) / 4) * (lv.sx / V);
+    return ((items + 127) / 128) * (long long)std::max(1, (lv.nz - 2 + 7) / 8 + 1);
+}
+
+void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done)
+{
+    count_launch(c);
+    const int V = c->es == 8 ? 2 : 4;
+    dim3 grid((unsigned)((lv.sp / V + 255) / 256), (unsigned)(lv.nz - 2));
+    if (c->es == 8) k_scale_rhs<double><<<grid, 256, 0, c->stream>>>(lp_of<double>(c, lv), (const double*)rhs, (double*)u, done);
+    else k_scale_rhs<float><<<grid, 256, 0, c->stream>>>(lp_of<float>(c, lv), (const float*)rhs, (float*)u, done);
+}
+
+template <typename T, bool HAS_RHS>
+static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
+{
+    constexpr int V = VN<T>::N;
+    constexpr int R = 4;
+    auto kern = k_resid_restrict_z<T, R, HAS_RHS>;
+    static int slots = 0;
+    if (!slots) {
+        int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
+        slots = std::max(1, nb) * c->num_sms;
+    }
+    const long long items = (long long)((f.sy + R - 1) / R) * (f.sx / V);
+    const long long warps = (items + 1 + 30) / 31;   // lanes 1..31 of each warp carry items
+    const long long xb = (warps + 3) / 4;
+    const int planes = co.nz - 2;
+    const int nzc = pick_chunks(xb, planes, slots, 4);
+    const int Kchunk = (planes + nzc - 1) / nzc;
+    const int nzc2 = (planes + Kchunk - 1) / Kchunk;
+    dim3 grid((unsigned)xb, (unsigned)nzc2);
+    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sp, co.nz, (T*)rc, Kchunk, nzc2, reverse, done);
+}
+
+void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
+{
+    count_launch(c);
+    if (c->es == 8) {
+        if (rhs) resid_restrict_t<double, true>(c, f, u, rhs, co, rc, reverse, done);
+        else resid_restrict_t<double, false>(c, f, u, rhs, co, rc, reverse, done);
+    } else {
+        if (rhs) resid_restrict_t<float, true>(c, f, u, rhs, co, rc, reverse, done);
+        else resid_restrict_t<float, false>(c, f, u, rhs, co, rc, reverse, done);
+    }
+}
+
+void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, const void* ec, int reverse, const int* done)
+{
+    count_launch(c);
+    const int V = c->es == 8 ? 2 : 4;
+    dim3 grid((unsigned)((f.sp / V + 255) / 256), (unsigned)(f.nz - 2));
+    if (c->es == 8)
+        k_prolong_v<double><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (double*)u, co.sx, co.sp, (const double*)ec, reverse, f.nz - 2, done);
+    else
+        k_prolong_v<float><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (float*)u, co.sx, co.sp, (const float*)ec, reverse, f.nz - 2, done);
+}
+
+}  // namespace mhs

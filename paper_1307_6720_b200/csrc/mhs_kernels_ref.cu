@@ -133,6 +133,10 @@ __global__ void __launch_bounds__(256) k_resnorm_partial_ref(LP<T> p, const T* _
 }
 
 // Deterministic final reduction + stop rule (C10): one block, fixed summation order.
+//   mode 1: the partials are the residual of the iterate reached after ctl->units completed cycles.
+//           units == 0: this is r0 (kept if the caller already knew it);  otherwise record cycle `units`
+//           and apply the stop rule.  If the solve goes on, units is advanced: the rest of the cycle may run.
+//   mode 2: r_last only (operator-level queries).
 __global__ void __launch_bounds__(1024) k_norm_final(const double* __restrict__ partial, long long n, Ctl* ctl, int mode)
 {
     if (mode == 1 && ctl->done) return;
@@ -141,26 +145,31 @@ __global__ void __launch_bounds__(1024) k_norm_final(const double* __restrict__ 
     v = block_sum<1024>(v);
     if (threadIdx.x == 0) {
         const double r = sqrt(v);
-        if (mode == 0) {
-            ctl->r0 = r;
-        } else if (mode == 1) {
-            const int k = ctl->cycles;
-            const double prev = k > 0 ? ctl->r_last : ctl->r0;
-            if (k < MHS_HISTORY_LEN) ctl->hist[k] = r;
-            ctl->cycles = k + 1;
+        if (mode == 2) {
             ctl->r_last = r;
-            const bool bad = !(r == r) || isinf(r);
-            if (bad) ctl->nan_seen = 1;
+            return;
+        }
+        const int k = ctl->units;
+        const bool bad = !(r == r) || isinf(r);
+        if (bad) ctl->nan_seen = 1;
+        if (k == 0) {
+            if (!(ctl->r0 > 0.0)) ctl->r0 = r;
+            ctl->r_last = r;
+            if (bad) ctl->done = 1;
+        } else {
+            const double prev = ctl->r_last;
+            if (k - 1 < MHS_HISTORY_LEN) ctl->hist[k - 1] = r;
+            ctl->cycles = k;
+            ctl->r_last = r;
             bool stag = false;
             if (ctl->stag_on) {  // C20: the fp32 residual floor shows as r_k > 0.9 r_{k-1} twice in a row
                 ctl->stag_count = (r > 0.9 * prev) ? ctl->stag_count + 1 : 0;
                 stag = ctl->stag_count >= 2;
                 if (stag) ctl->stagnated = 1;
             }
-            if (bad || stag || r <= ctl->tol * ctl->r0 || k + 1 >= ctl->max_cycles) ctl->done = 1;
-        } else {
-            ctl->r_last = r;
+            if (bad || stag || r <= ctl->tol * ctl->r0 || k >= ctl->max_cycles) ctl->done = 1;
         }
+        if (!ctl->done) ctl->units = k + 1;
     }
 }
 

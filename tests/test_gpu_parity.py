@@ -99,6 +99,12 @@ def test_operators_3d(B, orc, name, dtype, variant):
             S.level_set(3, lvl + 1, 0, dev(ec, dtype))
             S.op_prolong(3, lvl)
             assert relmax(host(S.level_get(3, lvl, 0)), orc.prolong_add3(ec, u3)) <= 2 * OPTOL[dtype]
+            # one whole V-cycle from this level (deeper levels start from zero, as inside a cycle)
+            u_in = u if lvl == 0 else np.zeros(shp)
+            S.level_set(3, lvl, 0, dev(u_in, dtype))
+            S.op_vcycle(3, lvl)
+            uv = orc.vcycle3(u_in, rhs, cl, w.alpha, Ll, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+            assert relmax(host(S.level_get(3, lvl, 0)), uv) <= 20 * OPTOL[dtype]
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
@@ -124,11 +130,12 @@ def test_operators_2d(B, orc, dtype):
             S.level_set(2, lvl + 1, 0, dev(ec, dtype))
             S.op_prolong(2, lvl)
             assert relmax(host(S.level_get(2, lvl, 0)), orc.prolong_add2(ec, u2)) <= 2 * OPTOL[dtype]
-            # one whole V-cycle from this level
-            S.level_set(2, lvl, 0, dev(u, dtype))
+            # one whole V-cycle from this level: level 0 continues from u, deeper levels start from
+            # zero exactly as they do inside a cycle (include/mhs.h: mhs_op_vcycle)
+            u_in = u if lvl == 0 else np.zeros(shp)
+            S.level_set(2, lvl, 0, dev(u_in, dtype))
             S.op_vcycle(2, lvl)
-            # the oracle's level rule counts from the level it is started on; pass the remaining depth
-            uv = orc.vcycle2(u, rhs, Ll, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+            uv = orc.vcycle2(u_in, rhs, Ll, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
             assert relmax(host(S.level_get(2, lvl, 0)), uv) <= 20 * OPTOL[dtype]
 
 
