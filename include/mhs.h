@@ -68,6 +68,8 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
 /* mhs_options.flags */
 #define MHS_FLAG_REFERENCE_KERNELS 1 /* one thread per node, one kernel per operator, no fusion: the
                                         paper's own kernel design; for A/B tests */
+#define MHS_FLAG_UNFUSED_KERNELS    4 /* tuned kernels, but one sweep per pass (no temporal blocking);
+                                        for A/B tests of the fused smoother                              */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 

@@ -166,8 +166,11 @@ mhs_status build_hierarchy(mhs_ctx* ctx, int dim, std::vector<Level>& Ls)
         const long long front = (dim == 3 ? lv.sp : 0) + lv.sx + 32;
         lv.pad = (front + 31) / 32 * 32;
         lv.alloc = lv.pad + lv.sp * nz + (dim == 3 ? lv.sp : 0) + lv.sx + 64;
-        // coefficient table: cx | cy | diag | w
-        std::vector<double> tab(4 * (size_t)nz);
+        // coefficient table: cx | cy | diag | w | A | Bx | By | Bz | iw | wz.  The last six are the per-plane
+        // coefficients of the expanded Jacobi update u' = A u + Bx (e+w) + By (n+s) + Bz (up+dn) + wz f used by
+        // the temporally blocked smoother (mhs_kernels_zfused.cu): A = 1-omega, Bx = -w cx, ..., iw = 1/w = D/omega;
+        // on the fixed planes k = 0 and k = nz-1 of a 3D level they read A = 1, B = 0, wz = 0: "copy through".
+        std::vector<double> tab(10 * (size_t)nz);
         for (int k = 0; k < nz; ++k) {
             const double cx = c[k] / (hx * hx), cy = c[k] / (hy * hy);
             const double d = -2.0 * cx - 2.0 * cy - (dim == 3 ? 2.0 / (hz * hz) : 0.0) + a2;
@@ -178,6 +181,14 @@ mhs_status build_hierarchy(mhs_ctx* ctx, int dim, std::vector<Level>& Ls)
                 return fail(ctx, MHS_ERR_INDEFINITE, b);
             }
             tab[k] = cx; tab[nz + k] = cy; tab[2 * nz + k] = d; tab[3 * nz + k] = ctx->opt.omega / d;
+            const double w = ctx->opt.omega / d;
+            const size_t n = (size_t)nz;
+            if (interior) {
+                tab[4 * n + k] = 1.0 - ctx->opt.omega; tab[5 * n + k] = -w * cx; tab[6 * n + k] = -w * cy;
+                tab[7 * n + k] = dim == 3 ? -w / (hz * hz) : 0.0; tab[8 * n + k] = 1.0 / w; tab[9 * n + k] = w;
+            } else {
+                tab[4 * n + k] = 1.0; tab[5 * n + k] = tab[6 * n + k] = tab[7 * n + k] = tab[8 * n + k] = tab[9 * n + k] = 0.0;
+            }
         }
         mhs_status st = upload(ctx, &lv.tab, tab);
         if (st) return st;
@@ -244,7 +255,12 @@ bool use_fast(const mhs_ctx* ctx, const Level& lv)
     return !(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fast_ok(ctx, lv);
 }
 
-int tail_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->tail3 : ctx->tail2; }
+bool use_zsweep(const mhs_ctx* ctx, const Level& lv)
+{
+    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && zsweep_ok(ctx, lv);
+}
+
+int clus_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->clus3 : ctx->clus2; }
 
 // `sweeps` Jacobi sweeps on level l, ping-ponging lv.u <-> lv.tmp.  want_norm: the first sweep also leaves
 // the partial sums of ||rhs - L u||^2 of ITS INPUT in ctx->partial (returned count; 0 = not computed).
@@ -254,6 +270,18 @@ long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const 
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
     const bool fast = use_fast(ctx, lv);
     long long npart = 0;
+    if (use_zsweep(ctx, lv)) {   // temporally blocked: two sweeps per pass over the iterate
+        for (int s = 0; s < sweeps;) {
+            const int S = std::min(2, sweeps - s);
+            Scope sc(ctx, kc_for(lv, l, 0));
+            const int n = launch_zsweep(ctx, lv, lv.u, rhs, lv.tmp, S, false, want_norm && s == 0, done);
+            if (want_norm && s == 0) npart = n;
+            std::swap(lv.u, lv.tmp);
+            if (lv.dim == 3 && l == 0) ctx->prof.sweeps_l0 += S;
+            s += S;
+        }
+        return npart;
+    }
     for (int s = 0; s < sweeps; ++s) {
         Scope sc(ctx, kc_for(lv, l, 0));
         if (fast) {
@@ -292,9 +320,9 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
 {
     Level& lv = Ls[l];
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
-    if (l > 0 && l >= tail_of(ctx, Ls)) {
+    if (l >= clus_of(ctx, Ls) && !lv.coarsest) {   // this level and everything below it: one cluster-kernel launch
         Scope sc(ctx, kc_for(lv, l, 0));
-        launch_tail(ctx, Ls, l, done);
+        launch_cluster(ctx, Ls, l, l == 0 ? 1 : 0, done);
         return;
     }
     if (lv.coarsest) {
@@ -305,9 +333,15 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
     Level& co = Ls[l + 1];
     const bool fast = use_fast(ctx, lv);
     int n_pre = ctx->opt.n_pre;
+    const bool zs = use_zsweep(ctx, lv);
     if (l > 0) {  // zero initial guess
         Scope sc(ctx, kc_for(lv, l, 0));
-        if (fast && n_pre >= 1) {
+        if (zs && n_pre >= 1) {
+            // the first sweep from zero is u = (omega/D) rhs: folded into the first temporally blocked pass
+            const int S = std::min(2, n_pre);
+            launch_zsweep(ctx, lv, nullptr, rhs, lv.u, S, true, false, done);
+            n_pre -= S;
+        } else if (fast && n_pre >= 1) {
             launch_scale_rhs(ctx, lv, rhs, lv.u, done);  // first sweep from zero: u = (omega/D) rhs
             n_pre -= 1;
         } else {
@@ -315,9 +349,10 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
         }
     }
     if (fuse_norm && l == 0) {
-        const long long np = smooth(ctx, Ls, l, 1, nullptr, true);  // must run even when `done` is about to be raised
+        const int first = zs ? std::min(2, n_pre) : 1;
+        const long long np = smooth(ctx, Ls, l, first, nullptr, true);  // must run even when `done` is about to be raised
         norm_final(ctx, lv, l, np, 1);
-        smooth(ctx, Ls, l, n_pre - 1, done);
+        smooth(ctx, Ls, l, n_pre - first, done);
     } else {
         smooth(ctx, Ls, l, n_pre, done);
     }
@@ -344,6 +379,23 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
     smooth(ctx, Ls, l, ctx->opt.n_post, done);
 }
 
+// Report a finished solve loop from the control block read back into ctx->ctl_host.
+mhs_status finish_cycles(mhs_ctx* ctx, double tol, mhs_solve_info* info)
+{
+    const Ctl* h = ctx->ctl_host;
+    if (info) {
+        info->cycles = h->cycles;
+        info->r0 = h->r0;
+        info->r_final = h->cycles > 0 ? h->r_last : h->r0;
+        info->stagnated = h->stagnated;
+        memset(info->history, 0, sizeof info->history);
+        memcpy(info->history, h->hist, sizeof(double) * std::min(h->cycles, MHS_HISTORY_LEN));
+    }
+    if (h->nan_seen) return fail(ctx, MHS_ERR_INDEFINITE, "residual norm is not finite (divergence: alpha^2 too large for the coarse grids?)");
+    if (!(h->r_last <= tol * h->r0) && !h->stagnated) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance");
+    return MHS_OK;
+}
+
 // Solve loop shared by the 2D and 3D drivers.  Unit q = [norm of iterate q-1 -> stop rule] + [V-cycle q];
 // units run speculatively in chunks behind the device-side stop flag and the host reads the control block
 // once per chunk.  The stop rule (C10) is exact: once the flag is up every later kernel returns at once, and
@@ -362,8 +414,21 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
     CK(cudaMemcpyAsync(ctx->ctl, h, sizeof(Ctl), cudaMemcpyHostToDevice, ctx->stream));
     Level& l0 = Ls[0];
     const int* done = &ctx->ctl->done;
-    const bool fuse = use_fast(ctx, l0) && ctx->opt.n_pre >= 1 && !l0.coarsest;
     const bool sync_each = (ctx->opt.flags & MHS_FLAG_SYNC_EACH_CYCLE) != 0;
+    if (clus_of(ctx, Ls) == 0 && !l0.coarsest && !sync_each) {
+        // The finest level is itself a cluster level: the whole solve loop runs in ONE kernel launch.
+        {
+            Scope sc(ctx, kc_for(l0, 0, 0));
+            launch_cluster(ctx, Ls, 0, 2, nullptr);
+        }
+        CK(cudaMemcpyAsync(h, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        drain_events(ctx);
+        CK(cudaGetLastError());
+        if ((h->cycles * (ctx->opt.n_pre + ctx->opt.n_post)) & 1) std::swap(l0.u, l0.tmp);
+        return finish_cycles(ctx, tol, info);
+    }
+    const bool fuse = use_fast(ctx, l0) && ctx->opt.n_pre >= 1 && !l0.coarsest && clus_of(ctx, Ls) > 0;
     std::vector<void*> iter_buf(1, l0.u);
     int issued = 0;
     bool trailing = false;
@@ -408,17 +473,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
         void* fin = iter_buf[h->cycles];
         if (fin != l0.u) std::swap(l0.u, l0.tmp);
     }
-    if (info) {
-        info->cycles = h->cycles;
-        info->r0 = h->r0;
-        info->r_final = h->cycles > 0 ? h->r_last : h->r0;
-        info->stagnated = h->stagnated;
-        memset(info->history, 0, sizeof info->history);
-        memcpy(info->history, h->hist, sizeof(double) * std::min(h->cycles, MHS_HISTORY_LEN));
-    }
-    if (h->nan_seen) return fail(ctx, MHS_ERR_INDEFINITE, "residual norm is not finite (divergence: alpha^2 too large for the coarse grids?)");
-    if (!(h->r_last <= tol * h->r0) && !h->stagnated) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance");
-    return MHS_OK;
+    return finish_cycles(ctx, tol, info);
 }
 
 mhs_status ensure_stage(mhs_ctx* ctx, size_t bytes)
@@ -555,8 +610,12 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
     ctx->tail3 = ref ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
     ctx->tail2 = ref ? (int)ctx->L2.size() : tail_start(ctx, ctx->L2, 216 * 1024);
-    ctx->npartial = std::max(resnorm_partial_capacity(ctx->L3[0]), resnorm_partial_capacity(ctx->L2[0]));
+    ctx->clus3 = ref ? (int)ctx->L3.size() : cluster_start(ctx, ctx->L3, ctx->tail3);
+    ctx->clus2 = ref ? (int)ctx->L2.size() : cluster_start(ctx, ctx->L2, ctx->tail2);
+    if (!ref) ctx->cluster_max = cluster_max_size(ctx);
+    ctx->npartial = std::max<long long>(64, std::max(resnorm_partial_capacity(ctx->L3[0]), resnorm_partial_capacity(ctx->L2[0])));
     for (const Level& lv : ctx->L3) ctx->npartial = std::max(ctx->npartial, smooth_z_partial_capacity(ctx, lv));
+    ctx->npartial = std::max<long long>(ctx->npartial, 4 * ctx->num_sms);
     CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
     CK(cudaMalloc((void**)&ctx->ctl, sizeof(Ctl)));
     CK(cudaMemset(ctx->ctl, 0, sizeof(Ctl)));

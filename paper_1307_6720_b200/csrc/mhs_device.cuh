@@ -49,4 +49,38 @@ __device__ __forceinline__ double block_sum(double v)
     return v;
 }
 
+// Stop rule (C10, C20), evaluated by ONE thread with the freshly reduced residual norm r.
+//   mode 1: r is the residual of the iterate reached after ctl->units completed cycles.
+//           units == 0: this is r0 (kept if the caller already knew it);  otherwise record cycle `units`
+//           and apply the stop rule.  If the solve goes on, units is advanced: the rest of the cycle may run.
+//   mode 2: r_last only (operator-level queries).
+__device__ __forceinline__ void stop_rule(Ctl* ctl, double r, int mode)
+{
+    if (mode == 2) {
+        ctl->r_last = r;
+        return;
+    }
+    const int k = ctl->units;
+    const bool bad = !(r == r) || isinf(r);
+    if (bad) ctl->nan_seen = 1;
+    if (k == 0) {
+        if (!(ctl->r0 > 0.0)) ctl->r0 = r;
+        ctl->r_last = r;
+        if (bad) ctl->done = 1;
+    } else {
+        const double prev = ctl->r_last;
+        if (k - 1 < MHS_HISTORY_LEN) ctl->hist[k - 1] = r;
+        ctl->cycles = k;
+        ctl->r_last = r;
+        bool stag = false;
+        if (ctl->stag_on) {  // C20: the fp32 residual floor shows as r_k > 0.9 r_{k-1} twice in a row
+            ctl->stag_count = (r > 0.9 * prev) ? ctl->stag_count + 1 : 0;
+            stag = ctl->stag_count >= 2;
+            if (stag) ctl->stagnated = 1;
+        }
+        if (bad || stag || r <= ctl->tol * ctl->r0 || k >= ctl->max_cycles) ctl->done = 1;
+    }
+    if (!ctl->done) ctl->units = k + 1;
+}
+
 }  // namespace mhs

@@ -78,7 +78,9 @@ struct mhs_ctx {
     mhs_profile prof{};
     int cur_kc = MHS_KC_PACK;  // kernel class the launchers charge
     int num_sms = 148;
-    int tail3 = 1 << 30, tail2 = 1 << 30;  // first level handled by the single-CTA tail kernel
+    int tail3 = 1 << 30, tail2 = 1 << 30;  // first level kept in shared memory by the cluster kernel's CTA 0
+    int clus3 = 1 << 30, clus2 = 1 << 30;  // first level handled by the cluster kernel (<= tail; mhs_kernels_cluster.cu)
+    int cluster_max = 8;                   // largest thread-block cluster the device co-schedules (<= 16)
     int dir = 0;               // z traversal direction of the next big kernel (alternates)
     std::vector<mhs::Ev> ev_pending;
     std::vector<cudaEvent_t> ev_pool;
@@ -113,7 +115,18 @@ long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);
 void launch_resid_restrict_z(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
 void launch_prolong_v(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, int reverse, const int* done);
+// ---- temporally blocked smoother (mhs_kernels_zfused.cu) ----
+bool zsweep_ok(const mhs_ctx* c, const Level& lv);
+// S (1 or 2) sweeps in one pass, u -> out.  zero: u is identically zero and not read.  norm: partial sums of the
+// squared residual of u go to c->partial; returns their number.
+int launch_zsweep(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, bool zero, bool norm, const int* done);
+
+// ---- the small-level cluster kernel (mhs_kernels_cluster.cu) ----
 int tail_start(const mhs_ctx* c, const std::vector<Level>& Ls, size_t budget_bytes);
-void launch_tail(mhs_ctx* c, std::vector<Level>& Ls, int l0, const int* done);
+int cluster_start(const mhs_ctx* c, const std::vector<Level>& Ls, int tail);
+int cluster_max_size(const mhs_ctx* c);
+// mode 0: V pass from level lc >= 1 with zero initial guess; 1: one V-cycle continuing from level 0 (lc == 0);
+// 2: the whole solve loop on level 0 (norm, stop rule in c->ctl, V-cycle) in one launch.
+void launch_cluster(mhs_ctx* c, std::vector<Level>& Ls, int lc, int mode, const int* done);
 
 }  // namespace mhs

@@ -1,0 +1,602 @@
+// The small-level kernel of libmhs_b200: ONE launch runs the whole lower part of the V-cycle -- every level
+// from the first one that is too small to fill the GPU down to the exact coarsest solve and back up -- on ONE
+// thread-block cluster, with hardware cluster barriers between the multigrid phases instead of kernel launches.
+//
+//   * "cluster levels" (a few hundred thousand nodes at most: they live in the L2) are worked on by all CTAs of
+//     the cluster out of global memory, one warp per row segment; a phase (sweep, residual, restriction,
+//     prolongation) ends in cluster.sync(), a ~0.2 us hardware barrier that also orders global memory.
+//   * "tail levels" (everything that fits in one SM's shared memory: u, rhs and a scratch array per level)
+//     are done by CTA 0 alone with __syncthreads() between the phases.
+//   * When the FINEST level of a hierarchy is itself a cluster level (the 2D boundary problem up to 513^2, the
+//     33^3 configuration) the kernel runs the whole SOLVE: residual norm, stop rule, V-cycle, repeated on the
+//     device until the stop rule fires -- one launch per mhs_solve_* call, no host round trip per cycle.
+//
+// On these levels the work is tiny and the paper's one-kernel-per-function design pays launch
+// latency ~25 times per level pair; this is what removes it.  Arithmetic: the same formulas as the reference
+// kernels (mhs_device.cuh), so the iterates are identical up to the order of the norm's summation.
+#include <cooperative_groups.h>
+
+#include <cstdio>
+#include <cstdlib>
+
+#include "mhs_device.cuh"
+
+namespace cg = cooperative_groups;
+
+namespace mhs {
+
+constexpr int CL_THREADS = 1024;
+constexpr int CL_MAXG = 4;             // cluster levels per launch
+constexpr long long CL_MAX_PTS = 600000;  // largest level given to the cluster instead of the whole GPU
+
+template <typename T>
+struct TailLevelP {
+    int nx, ny, nz;
+    int off_u, off_rhs, off_tmp;  // element offsets into the shared array
+    const T* tab;                 // global: cx | cy | diag | w
+    T cz;
+};
+
+template <typename T>
+struct GLevelP {                  // a cluster level: aliased Dirichlet layout in global memory
+    int nx, ny, nz, sx, sy, sp;
+    const T* tab;
+    T cz;
+    T *u, *tmp, *rhs, *r;         // rhs == nullptr: zero right-hand side (finest 3D level)
+};
+
+template <typename T>
+struct ClusterP {
+    int mode;                     // 0: V pass from level g[0] with zero initial guess; 1: one V-cycle continuing
+                                  // from g[0].u; 2: solve loop (norm, stop rule, V-cycle) on g[0]
+    int nglob, ntail, dim3, n_pre, n_post, ncoarse;
+    T a2;
+    GLevelP<T> g[CL_MAXG];
+    TailLevelP<T> t[8];
+    const T* ainv;                // global, ncoarse^2 (coarsest level, exact inverse)
+    const T* tail_rhs_g;          // top tail level, aliased layout (in)
+    T* tail_u_g;                  // top tail level, aliased layout (out)
+    int tail_sx, tail_sp;
+    double* partial;              // >= cluster size doubles
+    Ctl* ctl;
+};
+
+template <typename T>
+__device__ __forceinline__ T ldcg(const T* p) { return __ldcg(p); }
+
+// ---------------------------------------------------------------------------------------------
+// tail: levels in shared memory, plain dense layout (nx*ny*nz, walls stored as zeros), CTA 0 only
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ T tail_Lu(const TailLevelP<T>& L, const T* u, int i, int j, int k, bool d3, T a2)
+{
+    const int nx = L.nx, nxy = L.nx * L.ny;
+    const int c = i + nx * j + nxy * k;
+    const T uc = u[c];
+    T lu = L.tab[k] * lap1<T>(u[c + 1], u[c - 1], uc) + L.tab[L.nz + k] * lap1<T>(u[c + nx], u[c - nx], uc);
+    if (d3) lu += L.cz * lap1<T>(u[c + nxy], u[c - nxy], uc) + a2 * uc;
+    return lu;
+}
+
+template <typename T>
+__device__ void tail_body(const ClusterP<T>& P, T* S)
+{
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const bool d3 = P.dim3 != 0;
+    const int nlev = P.ntail;
+
+    // zero everything (walls must read as zeros), then load the top level's right-hand side
+    int tot = 0;
+    for (int l = 0; l < nlev; ++l) tot = max(tot, P.t[l].off_tmp + P.t[l].nx * P.t[l].ny * P.t[l].nz);
+    for (int q = tid; q < tot; q += nt) S[q] = T(0);
+    __syncthreads();
+    {
+        const TailLevelP<T>& L = P.t[0];
+        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
+        const int mx = L.nx - 2, my = L.ny - 2;
+        const int n = mx * my * (kz1 - kz0);
+        for (int q = tid; q < n; q += nt) {
+            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+            S[L.off_rhs + i + L.nx * j + L.nx * L.ny * k] = ldcg(P.tail_rhs_g + i + P.tail_sx * j + P.tail_sp * k);
+        }
+    }
+    __syncthreads();
+
+    // ---- down leg ----
+    for (int l = 0; l < nlev - 1; ++l) {
+        const TailLevelP<T>& L = P.t[l];
+        const TailLevelP<T>& C = P.t[l + 1];
+        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
+        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
+        T* u = S + L.off_u;
+        T* tmp = S + L.off_tmp;
+        const T* rhs = S + L.off_rhs;
+        for (int s = 0; s < P.n_pre; ++s) {
+            for (int q = tid; q < n; q += nt) {
+                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+                const int c = i + L.nx * j + L.nx * L.ny * k;
+                tmp[c] = u[c] + L.tab[3 * L.nz + k] * (rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2));
+            }
+            __syncthreads();
+            for (int q = tid; q < n; q += nt) {
+                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+                const int c = i + L.nx * j + L.nx * L.ny * k;
+                u[c] = tmp[c];
+            }
+            __syncthreads();
+        }
+        // residual -> tmp
+        for (int q = tid; q < n; q += nt) {
+            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+            const int c = i + L.nx * j + L.nx * L.ny * k;
+            tmp[c] = rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2);
+        }
+        __syncthreads();
+        // full weighting -> rhs of the next level
+        {
+            const int cmx = C.nx - 2, cmy = C.ny - 2;
+            const int ck0 = d3 ? 1 : 0, ck1 = d3 ? C.nz - 1 : 1;
+            const int cn = cmx * cmy * (ck1 - ck0);
+            T* rc = S + C.off_rhs;
+            for (int q = tid; q < cn; q += nt) {
+                const int I = q % cmx + 1, J = (q / cmx) % cmy + 1, K = q / (cmx * cmy) + ck0;
+                const T* r0 = tmp + 2 * I + L.nx * (2 * J) + L.nx * L.ny * (2 * K);
+                T s = T(0);
+                for (int dc = (d3 ? -1 : 0); dc <= (d3 ? 1 : 0); ++dc) {
+                    T sp = T(0);
+#pragma unroll
+                    for (int db = -1; db <= 1; ++db) {
+                        const T* row = r0 + L.nx * db + L.nx * L.ny * dc;
+                        const T sxv = T(0.25) * (row[-1] + row[1]) + T(0.5) * row[0];
+                        sp += (db == 0 ? T(0.5) : T(0.25)) * sxv;
+                    }
+                    s += (d3 ? (dc == 0 ? T(0.5) : T(0.25)) : T(1)) * sp;
+                }
+                rc[I + C.nx * J + C.nx * C.ny * K] = s;
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- coarsest level: exact solve e = A^-1 rhs (C9) ----
+    {
+        const TailLevelP<T>& L = P.t[nlev - 1];
+        const int mx = L.nx - 2, my = L.ny - 2, k0 = d3 ? 1 : 0;
+        const int n = P.ncoarse;
+        T* u = S + L.off_u;
+        const T* rhs = S + L.off_rhs;
+        for (int row = tid; row < n; row += nt) {
+            double s = 0.0;
+            for (int col = 0; col < n; ++col) {
+                const int ci = col % mx, cj = (col / mx) % my, ck = col / (mx * my);
+                s += (double)P.ainv[(long long)row * n + col] * (double)rhs[(ci + 1) + L.nx * (cj + 1) + L.nx * L.ny * (ck + k0)];
+            }
+            const int i = row % mx, j = (row / mx) % my, k = row / (mx * my);
+            u[(i + 1) + L.nx * (j + 1) + L.nx * L.ny * (k + k0)] = (T)s;
+        }
+        __syncthreads();
+    }
+
+    // ---- up leg ----
+    for (int l = nlev - 2; l >= 0; --l) {
+        const TailLevelP<T>& L = P.t[l];
+        const TailLevelP<T>& C = P.t[l + 1];
+        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
+        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
+        T* u = S + L.off_u;
+        T* tmp = S + L.off_tmp;
+        const T* rhs = S + L.off_rhs;
+        const T* ec = S + C.off_u;
+        for (int q = tid; q < n; q += nt) {
+            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+            const int I0 = i >> 1, I1 = (i + 1) >> 1, J0 = j >> 1, J1 = (j + 1) >> 1, K0 = k >> 1, K1 = (k + 1) >> 1;
+            const int cxy = C.nx * C.ny;
+            T s = (ec[I0 + C.nx * J0 + cxy * K0] + ec[I1 + C.nx * J0 + cxy * K0]) +
+                  (ec[I0 + C.nx * J1 + cxy * K0] + ec[I1 + C.nx * J1 + cxy * K0]);
+            if (d3)
+                s += (ec[I0 + C.nx * J0 + cxy * K1] + ec[I1 + C.nx * J0 + cxy * K1]) +
+                     (ec[I0 + C.nx * J1 + cxy * K1] + ec[I1 + C.nx * J1 + cxy * K1]);
+            u[i + L.nx * j + L.nx * L.ny * k] += (d3 ? T(0.125) : T(0.25)) * s;
+        }
+        __syncthreads();
+        for (int s = 0; s < P.n_post; ++s) {
+            for (int q = tid; q < n; q += nt) {
+                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+                const int c = i + L.nx * j + L.nx * L.ny * k;
+                tmp[c] = u[c] + L.tab[3 * L.nz + k] * (rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2));
+            }
+            __syncthreads();
+            for (int q = tid; q < n; q += nt) {
+                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+                const int c = i + L.nx * j + L.nx * L.ny * k;
+                u[c] = tmp[c];
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- write the correction of the top tail level back (interior nodes) ----
+    {
+        const TailLevelP<T>& L = P.t[0];
+        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
+        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
+        const T* u = S + L.off_u;
+        for (int q = tid; q < n; q += nt) {
+            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
+            P.tail_u_g[i + P.tail_sx * j + P.tail_sp * k] = u[i + L.nx * j + L.nx * L.ny * k];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// cluster levels: phases over global memory.  Work item = 32 consecutive interior nodes of one row;
+// items are dealt round-robin to all warps of the cluster.  Loads go through ld.global.cg: what one
+// CTA wrote in the previous phase must be seen by the others (L1 is not coherent across SMs).
+// ---------------------------------------------------------------------------------------------
+struct Who { int wg, nW, lane; };
+
+template <typename T, bool D3>
+struct RowIt {     // iterates the interior row segments of a level
+    int xch, nitems, sy1;
+    __device__ RowIt(int sx, int sy, int nz) : xch((sx - 1 + 31) / 32), sy1(sy - 1) { nitems = sy1 * (D3 ? nz - 2 : 1) * xch; }
+    __device__ __forceinline__ bool at(int it, int lane, int sx, int sp, int& i, int& j, int& k, int& idx) const
+    {
+        const int row = it / xch, c = it - row * xch;
+        const int kk = row / sy1, jj = row - kk * sy1;
+        i = 1 + 32 * c + lane; j = jj + 1; k = D3 ? kk + 1 : 0;
+        idx = i + sx * j + sp * k;
+        return i < sx;
+    }
+};
+
+template <typename T, bool D3>
+__device__ __forceinline__ T g_Lu(const GLevelP<T>& L, const T* __restrict__ u, int idx, int k, T a2)
+{
+    const T uc = ldcg(u + idx);
+    T lu = L.tab[k] * lap1<T>(ldcg(u + idx + 1), ldcg(u + idx - 1), uc) +
+           L.tab[L.nz + k] * lap1<T>(ldcg(u + idx + L.sx), ldcg(u + idx - L.sx), uc);
+    if (D3) lu += L.cz * lap1<T>(ldcg(u + idx + L.sp), ldcg(u + idx - L.sp), uc) + a2 * uc;
+    return lu;
+}
+
+// out = u + (omega/D_k) (rhs - L u)     (a2)
+template <typename T, bool D3>
+__device__ void ph_sweep(const GLevelP<T>& L, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ out, T a2, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+#pragma unroll 2
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+        const T f = rhs ? ldcg(rhs + idx) : T(0);
+        out[idx] = ldcg(u + idx) + L.tab[3 * L.nz + k] * (f - g_Lu<T, D3>(L, u, idx, k, a2));
+    }
+}
+
+// first sweep from the zero initial guess: u = (omega/D_k) rhs
+template <typename T, bool D3>
+__device__ void ph_scale(const GLevelP<T>& L, const T* __restrict__ rhs, T* __restrict__ out, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+#pragma unroll 2
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+        out[idx] = L.tab[3 * L.nz + k] * ldcg(rhs + idx);
+    }
+}
+
+template <typename T, bool D3>
+__device__ void ph_zero(const GLevelP<T>& L, T* __restrict__ out, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) out[idx] = T(0);
+    }
+}
+
+// r = rhs - L u   (a3)
+template <typename T, bool D3>
+__device__ void ph_residual(const GLevelP<T>& L, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ r, T a2, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+#pragma unroll 2
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+        const T f = rhs ? ldcg(rhs + idx) : T(0);
+        r[idx] = f - g_Lu<T, D3>(L, u, idx, k, a2);
+    }
+}
+
+// sum over interior nodes of (rhs - L u)^2 for this thread's items   (a7)
+template <typename T, bool D3>
+__device__ double ph_resnorm(const GLevelP<T>& L, const T* __restrict__ u, const T* __restrict__ rhs, T a2, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+    double acc = 0.0;
+#pragma unroll 2
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+        const T f = rhs ? ldcg(rhs + idx) : T(0);
+        const double r = (double)(f - g_Lu<T, D3>(L, u, idx, k, a2));
+        acc += r * r;
+    }
+    return acc;
+}
+
+// full weighting of r (fine, pitch fsx/fsp) into the coarse interior nodes   (a4)
+template <typename T, bool D3>
+__device__ void ph_restrict(const T* __restrict__ r, int fsx, int fsp, int csx, int csy, int cnz, int csp, T* __restrict__ rc, Who w)
+{
+    const RowIt<T, D3> R(csx, csy, cnz);
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int I, J, K, cidx;
+        if (!R.at(it, w.lane, csx, csp, I, J, K, cidx)) continue;
+        const T* q = r + 2 * I + fsx * (2 * J) + fsp * (2 * K);
+        T s = T(0);
+#pragma unroll
+        for (int dc = (D3 ? -1 : 0); dc <= (D3 ? 1 : 0); ++dc) {
+            T sp = T(0);
+#pragma unroll
+            for (int db = -1; db <= 1; ++db) {
+                const T* row = q + fsx * db + fsp * dc;
+                const T sxv = T(0.25) * (ldcg(row - 1) + ldcg(row + 1)) + T(0.5) * ldcg(row);
+                sp += (db == 0 ? T(0.5) : T(0.25)) * sxv;
+            }
+            s += (D3 ? (dc == 0 ? T(0.5) : T(0.25)) : T(1)) * sp;
+        }
+        rc[cidx] = s;
+    }
+}
+
+// u += P e_c  (tri/bi-linear, a6)
+template <typename T, bool D3>
+__device__ void ph_prolong(const GLevelP<T>& L, T* __restrict__ u, const T* __restrict__ ec, int csx, int csp, Who w)
+{
+    const RowIt<T, D3> R(L.sx, L.sy, L.nz);
+#pragma unroll 2
+    for (int it = w.wg; it < R.nitems; it += w.nW) {
+        int i, j, k, idx;
+        if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+        const int I0 = i >> 1, I1 = (i + 1) >> 1, J0 = j >> 1, J1 = (j + 1) >> 1, K0 = k >> 1, K1 = (k + 1) >> 1;
+        const T* a = ec + csp * K0;
+        T s = (ldcg(a + I0 + csx * J0) + ldcg(a + I1 + csx * J0)) + (ldcg(a + I0 + csx * J1) + ldcg(a + I1 + csx * J1));
+        if (D3) {
+            const T* b = ec + csp * K1;
+            s += (ldcg(b + I0 + csx * J0) + ldcg(b + I1 + csx * J0)) + (ldcg(b + I0 + csx * J1) + ldcg(b + I1 + csx * J1));
+        }
+        u[idx] = ldcg(u + idx) + (D3 ? T(0.125) : T(0.25)) * s;
+    }
+}
+
+template <typename T, bool D3>
+__global__ void __launch_bounds__(CL_THREADS, 1) k_cluster(const __grid_constant__ ClusterP<T> P, const int* __restrict__ done)
+{
+    if (P.mode != 2 && done && *done) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* S = reinterpret_cast<T*>(smem_raw);
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank(), ncta = (int)cluster.num_blocks();
+    Who w;
+    w.lane = threadIdx.x & 31;
+    w.wg = (threadIdx.x >> 5) * ncta + rank;   // interleave the CTAs: consecutive row segments go to different SMs
+    w.nW = ncta * (CL_THREADS / 32);
+    const int ng = P.nglob;
+
+    // current location of each cluster level's iterate (ping-pong)
+    T* cu[CL_MAXG];
+    T* ct[CL_MAXG];
+#pragma unroll
+    for (int l = 0; l < CL_MAXG; ++l) { cu[l] = P.g[l].u; ct[l] = P.g[l].tmp; }
+
+    for (;;) {
+        if (P.mode == 2) {
+            // ---- residual norm of the current iterate + stop rule (a7; C10) ----
+            double acc = ph_resnorm<T, D3>(P.g[0], cu[0], P.g[0].rhs, P.a2, w);
+            acc = block_sum<CL_THREADS>(acc);
+            if (threadIdx.x == 0) P.partial[rank] = acc;
+            cluster.sync();
+            if (rank == 0 && threadIdx.x == 0) {
+                double v = 0.0;
+                for (int q = 0; q < ncta; ++q) v += __ldcg(P.partial + q);
+                stop_rule(P.ctl, sqrt(v), 1);
+                __threadfence();
+            }
+            cluster.sync();
+            if (__ldcg(&P.ctl->done)) break;
+        }
+        // ---- down leg over the cluster levels ----
+#pragma unroll 1
+        for (int l = 0; l < ng; ++l) {
+            const GLevelP<T>& L = P.g[l];
+            int s0 = 0;
+            if (!(l == 0 && P.mode != 0)) {   // zero initial guess
+                if (P.n_pre >= 1) { ph_scale<T, D3>(L, L.rhs, cu[l], w); s0 = 1; }
+                else ph_zero<T, D3>(L, cu[l], w);
+                cluster.sync();
+            }
+            for (int s = s0; s < P.n_pre; ++s) {
+                ph_sweep<T, D3>(L, cu[l], L.rhs, ct[l], P.a2, w);
+                T* x = cu[l]; cu[l] = ct[l]; ct[l] = x;
+                cluster.sync();
+            }
+            ph_residual<T, D3>(L, cu[l], L.rhs, L.r, P.a2, w);
+            cluster.sync();
+            if (l + 1 < ng) {
+                const GLevelP<T>& C = P.g[l + 1];
+                ph_restrict<T, D3>(L.r, L.sx, L.sp, C.sx, C.sy, C.nz, C.sp, C.rhs, w);
+            } else {
+                const TailLevelP<T>& C = P.t[0];
+                ph_restrict<T, D3>(L.r, L.sx, L.sp, P.tail_sx, C.ny - 1, C.nz, P.tail_sp, const_cast<T*>(P.tail_rhs_g), w);
+            }
+            cluster.sync();
+        }
+        // ---- tail levels: CTA 0, shared memory ----
+        if (rank == 0) tail_body<T>(P, S);
+        if (ng > 0) cluster.sync();
+        // ---- up leg ----
+#pragma unroll 1
+        for (int l = ng - 1; l >= 0; --l) {
+            const GLevelP<T>& L = P.g[l];
+            if (l + 1 < ng) ph_prolong<T, D3>(L, cu[l], cu[l + 1], P.g[l + 1].sx, P.g[l + 1].sp, w);
+            else ph_prolong<T, D3>(L, cu[l], P.tail_u_g, P.tail_sx, P.tail_sp, w);
+            cluster.sync();
+            for (int s = 0; s < P.n_post; ++s) {
+                ph_sweep<T, D3>(L, cu[l], L.rhs, ct[l], P.a2, w);
+                T* x = cu[l]; cu[l] = ct[l]; ct[l] = x;
+                cluster.sync();
+            }
+        }
+        if (P.mode != 2) break;
+    }
+}
+
+// Which level can start the tail: the first level l >= 1 such that levels l.. fit in `budget` bytes.
+int tail_start(const mhs_ctx* c, const std::vector<Level>& Ls, size_t budget)
+{
+    const int n = (int)Ls.size();
+    for (int l = 1; l < n; ++l) {
+        if (n - l > 8) continue;  // at most 8 levels in the tail
+        size_t bytes = 0;
+        for (int q = l; q < n; ++q) bytes += 3 * (size_t)((Ls[q].npts() + 3) & ~3LL) * c->es;
+        if (bytes <= budget) return l;
+    }
+    return n;  // no tail
+}
+
+// First level handled by the cluster kernel: the cluster levels [result, tail) are those with at most
+// CL_MAX_PTS nodes (and at most CL_MAXG of them); result == tail means "tail only".
+int cluster_start(const mhs_ctx* c, const std::vector<Level>& Ls, int tail)
+{
+    const int n = (int)Ls.size();
+    if (tail >= n) return n;   // no tail -> no cluster kernel (the coarsest solve is part of the tail)
+    int l = tail;
+    while (l > 0 && tail - (l - 1) <= CL_MAXG && Ls[l - 1].npts() <= CL_MAX_PTS && Ls[l - 1].sp < (1LL << 30) / std::max(1, Ls[l - 1].nz)) --l;
+    return l;
+}
+
+// the opt-in dynamic shared memory limit is 227 KB minus the kernel's static shared memory
+template <typename K>
+static void set_cluster_attrs(K kern)
+{
+    cudaFuncAttributes fa;
+    size_t stat = 1024;
+    if (cudaFuncGetAttributes(&fa, kern) == cudaSuccess) stat = fa.sharedSizeBytes;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024 - stat));
+    cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    cudaGetLastError();
+}
+
+template <typename T, bool D3>
+static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, int mode, const int* done)
+{
+    ClusterP<T> P;
+    memset(&P, 0, sizeof P);
+    const int n = (int)Ls.size();
+    const int lt = std::max(lc, Ls[0].dim == 3 ? c->tail3 : c->tail2);   // lc > tail: a V pass from inside the tail
+    P.mode = mode;
+    P.nglob = lt - lc;
+    P.ntail = n - lt;
+    P.dim3 = D3;
+    P.n_pre = c->opt.n_pre; P.n_post = c->opt.n_post;
+    P.a2 = D3 ? (T)(c->alpha * c->alpha) : T(0);
+    for (int q = lc; q < lt; ++q) {
+        const Level& lv = Ls[q];
+        GLevelP<T>& g = P.g[q - lc];
+        g.nx = lv.nx; g.ny = lv.ny; g.nz = lv.nz; g.sx = lv.sx; g.sy = lv.sy; g.sp = (int)lv.sp;
+        g.tab = (const T*)lv.tab;
+        g.cz = D3 ? (T)(1.0 / (lv.hz * lv.hz)) : T(0);
+        g.u = (T*)lv.u; g.tmp = (T*)lv.tmp; g.rhs = (T*)lv.rhs; g.r = (T*)lv.r;
+    }
+    int off = 0;
+    for (int q = lt; q < n; ++q) {
+        const Level& lv = Ls[q];
+        TailLevelP<T>& t = P.t[q - lt];
+        t.nx = lv.nx; t.ny = lv.ny; t.nz = lv.nz;
+        const int npa = ((int)lv.npts() + 3) & ~3;
+        t.off_u = off; t.off_rhs = off + npa; t.off_tmp = off + 2 * npa;
+        off += 3 * npa;
+        t.tab = (const T*)lv.tab;
+        t.cz = D3 ? (T)(1.0 / (lv.hz * lv.hz)) : T(0);
+    }
+    P.ncoarse = Ls[n - 1].ncoarse;
+    P.ainv = (const T*)Ls[n - 1].ainv;
+    P.tail_rhs_g = (const T*)Ls[lt].rhs;
+    P.tail_u_g = (T*)Ls[lt].u;
+    P.tail_sx = Ls[lt].sx; P.tail_sp = (int)Ls[lt].sp;
+    P.partial = c->partial;
+    P.ctl = c->ctl;
+    const size_t smem = (size_t)off * sizeof(T);
+
+    auto kern = k_cluster<T, D3>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        set_cluster_attrs(kern);
+        attr_set = true;
+    }
+    int ncta = 1;
+    if (P.nglob > 0) {
+        // enough CTAs that a phase of the largest cluster level is a handful of row segments per warp
+        const long long items = Ls[lc].npts() / 32;
+        ncta = items > 4096 ? c->cluster_max : items > 1024 ? std::min(8, c->cluster_max) : items > 256 ? 4 : 2;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)ncta);
+    cfg.blockDim = dim3(CL_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)ncta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, P, done);
+    if (e != cudaSuccess || getenv("MHS_DEBUG"))
+        fprintf(stderr, "[mhs] k_cluster<%s,%dD> mode %d levels [%d,%d) tail [%d,%d) cluster %d smem %zu: %s\n", sizeof(T) == 8 ? "f64" : "f32",
+                D3 ? 3 : 2, mode, lc, lt, lt, n, ncta, smem, cudaGetErrorString(e));
+    return e;
+}
+
+// Largest cluster (<= 16 CTAs of CL_THREADS threads with the tail's shared memory) this device can co-schedule.
+int cluster_max_size(const mhs_ctx* c)
+{
+    (void)c;
+    int best = 1;
+    for (int n : {16, 8, 4, 2}) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)n); cfg.blockDim = dim3(CL_THREADS); cfg.dynamicSmemBytes = 216 * 1024;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)n; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        auto kern = k_cluster<double, true>;
+        set_cluster_attrs(kern);
+        int nc = 0;
+        if (cudaOccupancyMaxActiveClusters(&nc, kern, &cfg) == cudaSuccess && nc >= 1) { best = n; break; }
+        cudaGetLastError();
+    }
+    return best;
+}
+
+// mode 0: V pass from level lc >= 1 (zero initial guess); mode 1 / 2: lc == 0, one cycle / the whole solve.
+// Afterwards Ls[lc].u names the buffer that holds the result when the number of sweeps is known on the host
+// (modes 0 and 1); in mode 2 the caller fixes the names up from the cycle count (cluster_fix_names).
+void launch_cluster(mhs_ctx* c, std::vector<Level>& Ls, int lc, int mode, const int* done)
+{
+    count_launch(c);
+    cudaError_t e;
+    const bool d3 = Ls[0].dim == 3;
+    if (c->es == 8) e = d3 ? cluster_launch_t<double, true>(c, Ls, lc, mode, done) : cluster_launch_t<double, false>(c, Ls, lc, mode, done);
+    else e = d3 ? cluster_launch_t<float, true>(c, Ls, lc, mode, done) : cluster_launch_t<float, false>(c, Ls, lc, mode, done);
+    (void)e;   // surfaced by the caller's cudaGetLastError
+    const int lt = d3 ? c->tail3 : c->tail2;
+    if (lc < lt && mode != 2) {
+        const int np = c->opt.n_pre, nq = c->opt.n_post;
+        const int swaps = (mode == 0 ? (np >= 1 ? np - 1 : 0) : np) + nq;
+        if (swaps & 1) std::swap(Ls[lc].u, Ls[lc].tmp);
+    }
+}
+
+}  // namespace mhs

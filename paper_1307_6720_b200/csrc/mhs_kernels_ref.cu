@@ -132,45 +132,14 @@ __global__ void __launch_bounds__(256) k_resnorm_partial_ref(LP<T> p, const T* _
         partial[blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = v;
 }
 
-// Deterministic final reduction + stop rule (C10): one block, fixed summation order.
-//   mode 1: the partials are the residual of the iterate reached after ctl->units completed cycles.
-//           units == 0: this is r0 (kept if the caller already knew it);  otherwise record cycle `units`
-//           and apply the stop rule.  If the solve goes on, units is advanced: the rest of the cycle may run.
-//   mode 2: r_last only (operator-level queries).
+// Deterministic final reduction + stop rule (C10; stop_rule in mhs_device.cuh): one block, fixed summation order.
 __global__ void __launch_bounds__(1024) k_norm_final(const double* __restrict__ partial, long long n, Ctl* ctl, int mode)
 {
     if (mode == 1 && ctl->done) return;
     double v = 0.0;
     for (long long q = threadIdx.x; q < n; q += 1024) v += partial[q];
     v = block_sum<1024>(v);
-    if (threadIdx.x == 0) {
-        const double r = sqrt(v);
-        if (mode == 2) {
-            ctl->r_last = r;
-            return;
-        }
-        const int k = ctl->units;
-        const bool bad = !(r == r) || isinf(r);
-        if (bad) ctl->nan_seen = 1;
-        if (k == 0) {
-            if (!(ctl->r0 > 0.0)) ctl->r0 = r;
-            ctl->r_last = r;
-            if (bad) ctl->done = 1;
-        } else {
-            const double prev = ctl->r_last;
-            if (k - 1 < MHS_HISTORY_LEN) ctl->hist[k - 1] = r;
-            ctl->cycles = k;
-            ctl->r_last = r;
-            bool stag = false;
-            if (ctl->stag_on) {  // C20: the fp32 residual floor shows as r_k > 0.9 r_{k-1} twice in a row
-                ctl->stag_count = (r > 0.9 * prev) ? ctl->stag_count + 1 : 0;
-                stag = ctl->stag_count >= 2;
-                if (stag) ctl->stagnated = 1;
-            }
-            if (bad || stag || r <= ctl->tol * ctl->r0 || k >= ctl->max_cycles) ctl->done = 1;
-        }
-        if (!ctl->done) ctl->units = k + 1;
-    }
+    if (threadIdx.x == 0) stop_rule(ctl, sqrt(v), mode);
 }
 
 // dense (nx,ny,nz) -> internal layout.  Walls (i = 0, j = 0, top plane, and the bottom plane unless
