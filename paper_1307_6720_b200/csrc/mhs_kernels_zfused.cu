@@ -6,17 +6,19 @@
 //     of memory, so the input planes are brought in by the bulk-copy engine (cp.async.bulk global -> shared,
 //     completion on an mbarrier: the TMA data path without a tensor map) into a ring of NIN planes, several
 //     planes ahead of the arithmetic; no register or thread is spent on prefetching.
-//   * A CTA owns a tile of WY*R rows x TC columns and walks up in z.  Stage s of the pipeline lags one plane
+//   * A CTA owns a tile of WY*4 rows x TC columns and walks up in z.  Stage s of the pipeline lags one plane
 //     behind stage s-1: at step t stage 1 makes sweep-1 values of plane t-1 from the input planes t-2, t-1, t,
-//     stage 2 makes sweep-2 values of plane t-2 from sweep-1 planes t-3, t-2, t-1, ...  A thread keeps the z-column
-//     (below, centre) of its R x V nodes of every stage in registers; in-plane neighbours come from registers
-//     (rows of its own strip), warp shuffles (x) and a single shared-memory copy of the stage's centre plane.
-//   * Every stage shrinks the valid region by one row/plane at tile and chunk edges: a tile makes WY*R-2(S-1)
+//     stage 2 makes sweep-2 values of plane t-2 from sweep-1 planes t-3, t-2, t-1.  A thread owns a patch of
+//     4 rows x one 128-bit vector and keeps the z-column (below, centre, above) of its patch for every stage in
+//     registers; the step is unrolled three times so that the three register sets rotate by renaming, not by
+//     moves.  In-plane neighbours: rows of its own patch from registers, everything else from shared memory --
+//     the ring slot of the centre plane for stage 1, a double-buffered exchange plane for stage 2 -- with
+//     plain LDS (no shuffles, no lane-dependent branches).  One __syncthreads per plane.
+//   * Every stage shrinks the valid region by one row/plane at tile and chunk edges: a tile makes WY*4-2(S-1)
 //     output rows, a z-segment is warmed up over S planes.  Walls are held fixed in every stage; the bottom
 //     (data) and top planes pass through every stage by coefficients (A = 1, B = 0), so no branch is needed.
 //   * fp64 uses the expanded update  u' = (1-w) u + Bx (e+w) + By (n+s) + Bz (up+dn) + W f  with per-plane
-//     Bx = -(w/D) c/hx^2 ... : 7-8 DP instructions per update instead of 13 -- with S sweeps per byte the DP
-//     pipe (64 lanes/clk/SM), not HBM, would otherwise set the pace.  fp32 keeps the difference form (C20).
+//     Bx = -(w/D) c/hx^2 ... : 7 DP instructions per update.  fp32 keeps the difference form (C20).
 //   * The squared norm of the residual of the INPUT iterate is a by-product of stage 1 (r = (u'-u) D/w).
 //   * Work is a linearised list of (tile, plane) pairs cut into equal contiguous ranges, one per CTA, one CTA
 //     per SM: no wave quantisation whatever the grid size.
@@ -29,8 +31,11 @@
 namespace mhs {
 
 template <typename T> struct ZV;
-template <> struct ZV<double> { static constexpr int N = 2; };
-template <> struct ZV<float> { static constexpr int N = 4; };
+template <> struct ZV<double> { static constexpr int N = 2; static constexpr int NCO = 6; };
+template <> struct ZV<float> { static constexpr int N = 4; static constexpr int NCO = 4; };
+
+constexpr int ZR = 4;     // rows of a thread's patch
+constexpr int ZNIN = 4;   // input ring depth (planes)
 
 template <typename T>
 struct __align__(16) ZVec {
@@ -38,17 +43,24 @@ struct __align__(16) ZVec {
 };
 
 template <typename T>
+struct Patch {
+    ZVec<T> r[ZR];
+};
+
+template <typename T>
 struct ZP {
     int sx, sy, nz;
     long long sp;
     const T* tab;       // 10*nz: cx|cy|diag|w | A|Bx|By|Bz|iw|wz   (mhs_api.cu build_hierarchy)
-    T cz, a2;
+    T cz, a2, rho;      // 1/hz^2, alpha^2, Bx/By = hy^2/hx^2
     int WX, WY;         // warps per tile along x / y
     int TC, COUT, ntx;  // tile columns, output columns per tile, tiles along x (1: the tile is a full row)
-    int ROUT, nty;      // output rows per tile, tiles along y
+    int STEP, nty;      // distance between tiles along y (rows), tiles along y
     int NP;             // interior planes nz-2
     long long items;    // ntx*nty*NP
-    int nin;            // input ring depth
+    int zcap;           // planes of the shared coefficient table
+    int in_plane;       // elements of one ring slot: (WY*ZR + 2) rows x TC (also the size of an exchange plane)
+    int coef_bytes;     // bytes reserved for the coefficient table (multiple of 128)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -81,75 +93,247 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         : "memory");
 }
 
-__device__ __forceinline__ double zshfl_up(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
-__device__ __forceinline__ float zshfl_up(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
-__device__ __forceinline__ double zshfl_dn(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
-__device__ __forceinline__ float zshfl_dn(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
-
-template <typename T>
-struct Coef {   // per-plane coefficients of one sweep
-    T cx, cy, A, Bx, By, Bz, iw, wz;
-};
-
-template <typename T>
-__device__ __forceinline__ Coef<T> coef_at(const ZP<T>& p, int k)
-{
-    k = min(max(k, 0), p.nz - 1);
-    Coef<T> c;
-    const T* t = p.tab;
-    c.cx = t[k]; c.cy = t[p.nz + k];
-    c.A = t[4 * p.nz + k]; c.Bx = t[5 * p.nz + k]; c.By = t[6 * p.nz + k]; c.Bz = t[7 * p.nz + k];
-    c.iw = t[8 * p.nz + k]; c.wz = t[9 * p.nz + k];
-    return c;
-}
-
-// One Jacobi update of the V nodes of a vector.  c: centre values, cw/ce: the nodes left/right of the vector,
-// n/s: the rows above/below, up/dn: the planes above/below, f: right-hand side.  The fp32 version also returns
-// res = rhs - L u; in fp64 the caller recovers it from (out - c) * iw.
-template <bool HAS_RHS>
-__device__ __forceinline__ void jacobi_vec_d(const Coef<double>& k, const ZVec<double>& c, double cw, double ce, const ZVec<double>& n,
-                                             const ZVec<double>& s, const ZVec<double>& up, const ZVec<double>& dn, const ZVec<double>& f,
-                                             ZVec<double>& out)
-{
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-        const double w = e == 0 ? cw : c.v[0];
-        const double ea = e == 1 ? ce : c.v[1];
-        double o = k.A * c.v[e];
-        o = fma(k.Bx, ea + w, o);
-        o = fma(k.By, n.v[e] + s.v[e], o);
-        o = fma(k.Bz, up.v[e] + dn.v[e], o);
-        if (HAS_RHS) o = fma(k.wz, f.v[e], o);
-        out.v[e] = o;
-    }
-}
-
-template <bool HAS_RHS>
-__device__ __forceinline__ void jacobi_vec_f(const Coef<float>& k, float cz, float a2, const ZVec<float>& c, float cw, float ce,
-                                             const ZVec<float>& n, const ZVec<float>& s, const ZVec<float>& up, const ZVec<float>& dn,
-                                             const ZVec<float>& f, ZVec<float>& out, ZVec<float>& res)
-{
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const float w = e == 0 ? cw : c.v[e - 1];
-        const float ea = e == 3 ? ce : c.v[e + 1];
-        float lu = k.cx * lap1<float>(ea, w, c.v[e]) + k.cy * lap1<float>(n.v[e], s.v[e], c.v[e]);
-        lu += cz * lap1<float>(up.v[e], dn.v[e], c.v[e]) + a2 * c.v[e];
-        const float r = (HAS_RHS ? f.v[e] : 0.f) - lu;
-        res.v[e] = r;
-        out.v[e] = c.v[e] + k.wz * r;
-    }
-}
-
 template <typename T>
 __device__ __forceinline__ ZVec<T> zld(const T* p) { return *reinterpret_cast<const ZVec<T>*>(p); }
 template <typename T>
 __device__ __forceinline__ void zst(T* p, const ZVec<T>& a) { *reinterpret_cast<ZVec<T>*>(p) = a; }
 
+// Per-plane coefficients of one sweep (warp-uniform, read from the shared table).
+//   fp64 (expanded update):  u' = A u + By (rho (e+w) + (n+s)) + Bz (up+dn) + wz f ;  iw2 = (D/omega)^2 for the norm
+//   fp32 (difference form):  u' = u + wz (f - L u) with cx, cy per plane
+template <typename T> struct ZCoef;
+template <> struct ZCoef<double> {
+    double A, By, Bz, wz, iw2;
+    __device__ __forceinline__ void load(const double* ck, bool rhs, bool norm)
+    {
+        const double2 a = *reinterpret_cast<const double2*>(ck);
+        const double2 b = *reinterpret_cast<const double2*>(ck + 2);
+        A = a.x; By = a.y; Bz = b.x; wz = rhs ? b.y : 0.0;
+        iw2 = norm ? ck[4] : 0.0;
+    }
+};
+template <> struct ZCoef<float> {
+    float cx, cy, wz;
+    __device__ __forceinline__ void load(const float* ck, bool, bool)
+    {
+        const float4 a = *reinterpret_cast<const float4*>(ck);
+        cx = a.x; cy = a.y; wz = a.z;
+    }
+};
+
+__device__ __forceinline__ double zc_iw2(const ZCoef<double>& k) { return k.iw2; }
+__device__ __forceinline__ double zc_iw2(const ZCoef<float>&) { return 0.0; }
+
+// One Jacobi update of one row of a thread's patch.  c: the row's centre values, w/e: the elements left / right of
+// the vector, n/s: the rows above / below, up/dn: the planes above / below, f: right-hand side.  rs (fp32 only): the
+// sum of the squared residuals of the row, without element 0 when it is a wall (cw0).
+template <bool HAS_RHS>
+__device__ __forceinline__ void jac_row(const ZCoef<double>& k, double rho, double, double, const ZVec<double>& c, double w, double e,
+                                        const ZVec<double>& n, const ZVec<double>& s, const ZVec<double>& up, const ZVec<double>& dn,
+                                        const ZVec<double>& f, ZVec<double>& o, bool, float&)
+{
+    double o0 = k.A * c.v[0], o1 = k.A * c.v[1];
+    const double h0 = fma(rho, c.v[1] + w, n.v[0] + s.v[0]);
+    const double h1 = fma(rho, e + c.v[0], n.v[1] + s.v[1]);
+    o0 = fma(k.By, h0, o0);
+    o1 = fma(k.By, h1, o1);
+    o0 = fma(k.Bz, up.v[0] + dn.v[0], o0);
+    o1 = fma(k.Bz, up.v[1] + dn.v[1], o1);
+    if (HAS_RHS) {
+        o0 = fma(k.wz, f.v[0], o0);
+        o1 = fma(k.wz, f.v[1], o1);
+    }
+    o.v[0] = o0;
+    o.v[1] = o1;
+}
+
+template <bool HAS_RHS>
+__device__ __forceinline__ void jac_row(const ZCoef<float>& k, float, float cz, float a2, const ZVec<float>& c, float w, float e,
+                                        const ZVec<float>& n, const ZVec<float>& s, const ZVec<float>& up, const ZVec<float>& dn,
+                                        const ZVec<float>& f, ZVec<float>& o, bool cw0, float& rs)
+{
+    float ra = 0.f;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float cc = c.v[q];
+        const float ww = q == 0 ? w : c.v[q - 1 < 0 ? 0 : q - 1];
+        const float ee = q == 3 ? e : c.v[q + 1 > 3 ? 3 : q + 1];
+        float lu = k.cx * lap1<float>(ee, ww, cc) + k.cy * lap1<float>(n.v[q], s.v[q], cc);
+        lu += cz * lap1<float>(up.v[q], dn.v[q], cc) + a2 * cc;
+        const float res = (HAS_RHS ? f.v[q] : 0.f) - lu;
+        if (q > 0 || !cw0) ra = fmaf(res, res, ra);   // a wall element has no residual
+        o.v[q] = cc + k.wz * res;
+    }
+    rs = ra;
+}
+
 // ------------------------------------------------------------------------------------------------
 // S sweeps.  ZERO: the input iterate is identically zero (coarse-grid correction, first pre-sweep):
 // sweep 1 is u = (omega/D) rhs and no input plane is read at all.
 // ------------------------------------------------------------------------------------------------
+template <typename T>
+struct ZCtx {
+    const T* __restrict__ rhs;    // plane 0 of the right-hand side (uniform)
+    T* __restrict__ out;          // plane 0 of the output (uniform)
+    unsigned own;                 // in-plane offset of (patch row 0, element 0)
+    uint32_t bars;                // shared-space address of the mbarriers
+    const T* coef;                // shared: coefficient records, plane kstart first
+    const T* in_own;              // shared: ring slot 0 + offset of the patch
+    T* ex_own;                    // shared: exchange plane 0 + offset of the patch
+    const T* tile_src;            // global: (first tile row, first tile column) of plane 0
+    int kstart, kend_in, kb, ke;
+    int nload, nwait, knext, stepc;
+    int omask;                    // rows of the patch that are stored (output rows, output columns)
+    bool cw0;                     // element 0 of the patch is a wall column
+    double acc;
+};
+
+template <typename T>
+__device__ __forceinline__ void z_issue(const ZP<T>& p, ZCtx<T>& z, T* IN, int k)
+{
+    // warp 0: request input plane k into ring slot nload % ZNIN
+    const int slot = z.nload & (ZNIN - 1);
+    T* dst = IN + (size_t)slot * p.in_plane;
+    const T* src = z.tile_src + p.sp * k;
+    const uint32_t plane_bytes = (uint32_t)p.in_plane * sizeof(T);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + slot;
+    const int lane = threadIdx.x & 31;
+    if (p.ntx == 1) {
+        if (lane == 0) {
+            mbar_expect_tx(bar, plane_bytes);
+            bulk_g2s(dst, src, plane_bytes, bar);
+        }
+    } else {
+        if (lane == 0) mbar_expect_tx(bar, plane_bytes);
+        __syncwarp();
+        const int rows_in = p.WY * ZR + 2;
+        for (int r = lane; r < rows_in; r += 32)
+            bulk_g2s(dst + r * p.TC, src + (long long)r * p.sx, (uint32_t)(p.TC * sizeof(T)), bar);
+    }
+}
+
+// End of a plane step: the ring slot of plane t-1 and the exchange plane of t-2 have been read by everybody.
+template <typename T, bool ZERO>
+__device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, T* IN, int t, bool fresh)
+{
+    __syncthreads();
+    if (!ZERO) {
+        if (fresh) ++z.nwait;
+        if (t > z.kstart && z.knext <= z.kend_in) {   // the slot of plane t-1 is free: request the next plane into it
+            if (threadIdx.x < 32) z_issue(p, z, IN, z.knext);
+            ++z.nload;
+            ++z.knext;
+        }
+    }
+    ++z.stepc;
+}
+
+// First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
+template <typename T, bool ZERO>
+__device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, T* IN, Patch<T>& dn0, int t)
+{
+    if (!ZERO) {
+        const T* newp = z.in_own + (size_t)(z.nwait & (ZNIN - 1)) * p.in_plane;
+        uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + (z.nwait & (ZNIN - 1));
+        mbar_wait(bar, (uint32_t)((z.nwait / ZNIN) & 1));
+#pragma unroll
+        for (int r = 0; r < ZR; ++r) dn0.r[r] = zld(newp + r * p.TC);
+    }
+    z_advance<T, ZERO>(p, z, IN, t, true);
+}
+
+// One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
+// slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
+// caller swaps the names (the step is unrolled twice), so no register is ever moved.
+template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
+__device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1, const Patch<T>& c1,
+                                       int t)
+{
+    constexpr int V = ZV<T>::N;
+    constexpr int NCO = ZV<T>::NCO;
+    const int TC = p.TC;
+    const int p1 = t - 1, p2 = t - 2;                  // p1 >= kstart >= 0; p2 >= -1
+    const bool in1 = p1 >= z.kb && p1 < z.ke;          // plane p1 is an output plane of this segment
+    const bool in2 = p2 >= z.kb && p2 < z.ke;
+    const bool fresh = !ZERO && t <= z.kend_in;        // a new input plane arrives in this step
+    // !fresh (only the step after the top plane): the slot holds an older plane -- finite numbers that meet Bz = 0
+    const T* newp = z.in_own + (size_t)(z.nwait & (ZNIN - 1)) * p.in_plane;          // plane t
+    const T* cenp = z.in_own + (size_t)((z.nwait - 1) & (ZNIN - 1)) * p.in_plane;    // plane t-1
+    T* exw = z.ex_own + (size_t)(z.stepc & 1) * p.in_plane;                            // sweep-1 plane t-1 (written now)
+    const T* exr = z.ex_own + (size_t)((z.stepc & 1) ^ 1) * p.in_plane;                // sweep-1 plane t-2 (written a step ago)
+    if (fresh) {
+        uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + (z.nwait & (ZNIN - 1));
+        mbar_wait(bar, (uint32_t)((z.nwait / ZNIN) & 1));
+    }
+    ZCoef<T> k1, k2;
+    k1.load(z.coef + (p1 - z.kstart) * NCO, HAS_RHS, NORM);
+    if (S == 2) k2.load(z.coef + max(p2 - z.kstart, 0) * NCO, HAS_RHS, false);
+    // uniform plane bases + 32-bit per-thread offsets
+    const T* f1p = HAS_RHS ? z.rhs + p.sp * p1 : nullptr;
+    const T* f2p = HAS_RHS ? z.rhs + p.sp * max(p2, 0) : nullptr;
+    T* o1p = z.out + p.sp * p1;
+    T* o2p = z.out + p.sp * max(p2, 0);
+    const int m1 = in1 ? z.omask : 0, m2 = in2 ? z.omask : 0;
+    ZVec<T> s1, n1, s2, n2;
+    if (!ZERO) { s1 = zld(cenp - TC); n1 = zld(cenp + ZR * TC); }
+    if (S == 2) { s2 = zld(exr - TC); n2 = zld(exr + ZR * TC); }
+    double pa = 0.0;
+    float pf = 0.f;
+#pragma unroll
+    for (int r = 0; r < ZR; ++r) {
+        const unsigned goff = z.own + (unsigned)r * (unsigned)p.sx;
+        // ---------------- stage 1: sweep-1 values of row r of plane t-1 ----------------
+        ZVec<T> up0, o1, f1;
+        if (!ZERO) up0 = zld(newp + r * TC);
+        if (HAS_RHS) f1 = zld(f1p + goff);
+        if (ZERO) {
+#pragma unroll
+            for (int e = 0; e < V; ++e) o1.v[e] = k1.wz * f1.v[e];
+            if (z.cw0) o1.v[0] = T(0);
+        } else {
+            const T w = cenp[r * TC - 1], e = cenp[r * TC + V];
+            const ZVec<T>& nn = r == ZR - 1 ? n1 : c0.r[r + 1 < ZR ? r + 1 : r];
+            const ZVec<T>& ss = r == 0 ? s1 : c0.r[r > 0 ? r - 1 : 0];
+            float rs = 0.f;
+            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], w, e, nn, ss, up0, dn0.r[r], f1, o1, z.cw0, rs);
+            if (z.cw0) o1.v[0] = c0.r[r].v[0];
+            if (NORM && (m1 & (1 << r))) {
+                if (sizeof(T) == 8) {
+#pragma unroll
+                    for (int q = 0; q < V; ++q) {
+                        const double d = (double)o1.v[q] - (double)c0.r[r].v[q];
+                        pa = fma(d, d, pa);
+                    }
+                } else {
+                    pf += rs;
+                }
+            }
+            dn0.r[r] = up0;     // becomes the centre plane of the next step
+        }
+        if (S == 1) {
+            if (m1 & (1 << r)) zst(o1p + goff, o1);
+        } else {
+            zst(exw + r * TC, o1);
+            // ---------------- stage 2: sweep-2 values of row r of plane t-2 ----------------
+            ZVec<T> o2, f2;
+            if (HAS_RHS) f2 = zld(f2p + goff);
+            const T w = exr[r * TC - 1], e = exr[r * TC + V];
+            const ZVec<T>& nn = r == ZR - 1 ? n2 : c1.r[r + 1 < ZR ? r + 1 : r];
+            const ZVec<T>& ss = r == 0 ? s2 : c1.r[r > 0 ? r - 1 : 0];
+            float rs;
+            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], w, e, nn, ss, o1, dn1.r[r], f2, o2, false, rs);
+            if (z.cw0) o2.v[0] = c1.r[r].v[0];
+            if (m2 & (1 << r)) zst(o2p + goff, o2);
+            dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
+        }
+    }
+    if (NORM) {
+        if (sizeof(T) == 8) z.acc = fma(zc_iw2(k1), pa, z.acc);   // pa == 0 unless plane p1 is an output plane
+        else z.acc += (double)pf;
+    }
+    z_advance<T, ZERO>(p, z, IN, t, fresh);
+}
+
 template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
 __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
@@ -158,226 +342,127 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
     static_assert(!ZERO || HAS_RHS, "a zero iterate with a zero right-hand side stays zero");
     if (done && *done) return;
     constexpr int V = ZV<T>::N;
-    constexpr int R = 4;
+    constexpr int NCO = ZV<T>::NCO;
+    constexpr int H = S - 1;                               // rows a tile loses on each side to the later sweeps
     extern __shared__ __align__(128) unsigned char zsm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wx = warp % p.WX, wy = warp / p.WX;
     const int TC = p.TC;
-    const int rows_in = p.WY * R + 2;                       // input tile: one halo row below and above
-    const int in_plane = rows_in * TC;                      // elements
-    // shared memory: [mbarriers: 8 x 8 B, padded to 128] [IN ring: nin planes] [EX: (WY*R + 2) rows, guard row each side]
+    const int NR = p.WY * ZR;                              // patch rows of a tile
+    // shared memory: [mbarriers: 128 B] [coefficients] [IN ring: ZNIN planes] [EX: 2 exchange planes]
     uint64_t* bars = reinterpret_cast<uint64_t*>(zsm);
-    T* IN = reinterpret_cast<T*>(zsm + 128);
-    T* EX = IN + (size_t)(ZERO ? 0 : p.nin) * in_plane + TC;   // -> row 0 of the exchange tile (guard row before it)
+    T* coef = reinterpret_cast<T*>(zsm + 128);
+    T* IN = reinterpret_cast<T*>(zsm + 128 + p.coef_bytes);
+    T* EX = IN + (size_t)(ZERO ? 0 : ZNIN) * p.in_plane;
 
     if (!ZERO && threadIdx.x == 0) {
-        for (int q = 0; q < p.nin; ++q) mbar_init(bars + q, 1);
+        for (int q = 0; q < ZNIN; ++q) mbar_init(bars + q, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (S == 2) {   // guard rows and never-written parts of the exchange planes must hold zeros (a wall row may sit there)
+        for (int q = threadIdx.x; q < 2 * p.in_plane; q += blockDim.x) EX[q] = T(0);
     }
     __syncthreads();
 
     const int cx0 = (wx * 32 + lane) * V;                   // first column of this thread's vector inside the tile
+    ZCtx<T> z;
+    z.rhs = rhs;
+    z.out = out;
+    z.bars = smem_u32(bars);
+    z.coef = coef;
+    z.in_own = IN + (wy * ZR + 1) * TC + cx0;
+    z.ex_own = EX + (wy * ZR + 1) * TC + cx0;
+    z.nload = 0;                                            // planes requested so far by this CTA (ring position)
+    z.nwait = 0;                                            // planes consumed so far
+    z.stepc = 0;
+    z.acc = 0.0;
     const long long q0 = p.items * blockIdx.x / gridDim.x, q1 = p.items * (blockIdx.x + 1) / gridDim.x;
-    int nload = 0;                                          // planes requested so far by this CTA (ring position)
-    int nwait = 0;                                          // planes consumed so far
-    double acc = 0.0;
 
     for (long long q = q0; q < q1;) {
         const int tile = (int)(q / p.NP);
-        const int kb = 1 + (int)(q - (long long)tile * p.NP);
-        const int ke = (int)min((long long)p.NP + 1, kb + (q1 - q));   // output planes [kb, ke)
-        q += ke - kb;
+        z.kb = 1 + (int)(q - (long long)tile * p.NP);
+        z.ke = (int)min((long long)p.NP + 1, z.kb + (q1 - q));   // output planes [kb, ke)
+        q += z.ke - z.kb;
         const int ty = tile / p.ntx, tx = tile - ty * p.ntx;
         const int ct = p.ntx == 1 ? 0 : tx * p.COUT - V;              // first column of the tile
-        const int jt = ty * p.ROUT - (S - 1);                          // first row of the strips
-        const int kstart = max(kb - S, 0), kend_in = min(ke - 1 + S, p.nz - 1);
-        const T* tile_src = u + (long long)(jt - 1) * p.sx + ct;      // (row jt-1, col ct) of plane 0
-        const uint32_t plane_bytes = (uint32_t)in_plane * sizeof(T);
+        // Tiles along y: patch rows [jt, jt+NR) are interior rows; the wall rows j = 0 / j = sy are only ever
+        // read -- from the input halo row in sweep 1, from the (zero) guard row of the exchange plane in sweep 2.
+        const int jt = min(1 + ty * p.STEP, p.sy - NR);                // first patch row
+        const int jlo = ty == 0 ? 1 : 1 + ty * p.STEP + H;             // rows [jlo, jhi) are this tile's output
+        const int jhi = ty == p.nty - 1 ? p.sy : 1 + ty * p.STEP + NR - H;
+        z.kstart = max(z.kb - S, 0);
+        z.kend_in = min(z.ke - 1 + S, p.nz - 1);
+        z.tile_src = u + (long long)(jt - 1) * p.sx + ct;             // (row jt-1, col ct) of plane 0
 
-        auto issue = [&](int k) {   // warp 0: request input plane k into ring slot nload % nin
-            const int slot = nload % p.nin;
-            T* dst = IN + (size_t)slot * in_plane;
-            const T* src = tile_src + p.sp * k;
-            if (lane == 0) mbar_expect_tx(bars + slot, plane_bytes);
-            __syncwarp();
-            if (p.ntx == 1) {
-                if (lane == 0) bulk_g2s(dst, src, plane_bytes, bars + slot);
+        // per-plane coefficient records of this segment
+        __syncthreads();   // the previous segment is done with the table
+        for (int i = threadIdx.x; i < (z.kend_in - z.kstart + 1) * NCO; i += blockDim.x) {
+            const int k = z.kstart + i / NCO, c = i % NCO;
+            const T* t = p.tab;
+            T v = T(0);
+            if (sizeof(T) == 8) {
+                // A | By | Bz | wz | iw^2 | -
+                if (c == 0) v = t[4 * p.nz + k];
+                else if (c == 1) v = t[6 * p.nz + k];
+                else if (c == 2) v = t[7 * p.nz + k];
+                else if (c == 3) v = t[9 * p.nz + k];
+                else if (c == 4) v = t[8 * p.nz + k] * t[8 * p.nz + k];
             } else {
-                for (int r = lane; r < rows_in; r += 32) bulk_g2s(dst + r * TC, src + (long long)r * p.sx, (uint32_t)(TC * sizeof(T)), bars + slot);
+                // cx | cy | wz | -
+                if (c < 2) v = t[c * p.nz + k];
+                else if (c == 2) v = t[9 * p.nz + k];
             }
-        };
-        int knext = kstart;     // next plane to request
+            coef[i] = v;
+        }
+
+        z.knext = z.kstart;     // next plane to request
         if (!ZERO) {
-            if (warp == 0)
-                for (int n = 0; n < p.nin && knext + n <= kend_in; ++n) { issue(knext + n); ++nload; }
-            else
-                nload += min(p.nin, kend_in - knext + 1);
-            knext += min(p.nin, kend_in - knext + 1);
+            const int n = min(ZNIN, z.kend_in - z.knext + 1);
+            for (int i = 0; i < n; ++i) {
+                if (warp == 0) z_issue(p, z, IN, z.knext + i);
+                ++z.nload;
+            }
+            z.knext += n;
         }
+        __syncthreads();   // coefficient table visible
 
-        // wall / validity masks of this thread's nodes
-        const int jrow0 = jt + wy * R;                                  // grid row of strip row 0
+        // wall / validity masks of this thread's patch
+        const int jrow0 = jt + wy * ZR;                                 // grid row of patch row 0
         const int icol0 = ct + cx0;                                     // grid column of vector element 0
-        bool colwall[V];
-#pragma unroll
-        for (int e = 0; e < V; ++e) colwall[e] = (icol0 + e == 0) || (icol0 + e == p.sx);
+        z.cw0 = (icol0 == 0) || (icol0 == p.sx);
         const bool col_out = p.ntx == 1 ? true : (cx0 >= V && cx0 < TC - V && icol0 < p.sx);
-        bool rowwall[R], row_out[R];
+        z.omask = 0;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
+        for (int r = 0; r < ZR; ++r) {
             const int j = jrow0 + r;
-            rowwall[r] = (j == 0) || (j == p.sy);
-            const int jo = j - ty * p.ROUT;
-            row_out[r] = jo >= 0 && jo < p.ROUT && j > 0 && j < p.sy;
+            if (col_out && j >= jlo && j < jhi) z.omask |= 1 << r;
         }
+        // in-plane offset of (patch row 0, element 0).  jrow0 >= 1; icol0 >= -V only for halo vectors of the first
+        // x tile, which neither load nor store through it: clamp
+        z.own = (unsigned)(jrow0 * p.sx + max(icol0, 0));
 
-        ZVec<T> cm0[R], cc0[R], cm1[R], cc1[R], fprev[R];
+        Patch<T> X, Y, P, Q;
 #pragma unroll
-        for (int r = 0; r < R; ++r)
+        for (int r = 0; r < ZR; ++r)
 #pragma unroll
-            for (int e = 0; e < V; ++e) { cm0[r].v[e] = cc0[r].v[e] = cm1[r].v[e] = cc1[r].v[e] = fprev[r].v[e] = T(0); }
+            for (int e = 0; e < V; ++e) X.r[r].v[e] = Y.r[r].v[e] = P.r[r].v[e] = Q.r[r].v[e] = T(0);
 
-        const long long own = (long long)jrow0 * p.sx + icol0;          // in-plane offset of (strip row 0, element 0)
-
-        for (int t = kstart; t <= ke - 1 + S; ++t) {
-            // ---------------- stage 1: sweep-1 values of plane t-1 ----------------
-            const int p1 = t - 1;
-            const bool act1 = p1 >= kstart && p1 <= kend_in;
-            ZVec<T> cp0[R], u1[R], f1[R];
-            if (!ZERO) {
-                if (t <= kend_in) {
-                    const int slot = nwait % p.nin;
-                    mbar_wait(bars + slot, (uint32_t)((nwait / p.nin) & 1));
-                    const T* pin = IN + (size_t)slot * in_plane + (wy * R + 1) * TC + cx0;
-#pragma unroll
-                    for (int r = 0; r < R; ++r) cp0[r] = zld(pin + r * TC);
-                } else {
-#pragma unroll
-                    for (int r = 0; r < R; ++r)
-#pragma unroll
-                        for (int e = 0; e < V; ++e) cp0[r].v[e] = T(0);
-                }
-            }
-            if (HAS_RHS && act1) {
-#pragma unroll
-                for (int r = 0; r < R; ++r) f1[r] = zld(rhs + own + p.sp * p1 + (long long)r * p.sx);
-            } else {
-#pragma unroll
-                for (int r = 0; r < R; ++r)
-#pragma unroll
-                    for (int e = 0; e < V; ++e) f1[r].v[e] = T(0);
-            }
-            if (ZERO) {
-                const Coef<T> k1 = coef_at(p, p1);
-#pragma unroll
-                for (int r = 0; r < R; ++r)
-#pragma unroll
-                    for (int e = 0; e < V; ++e) u1[r].v[e] = (rowwall[r] || colwall[e] || !act1) ? T(0) : k1.wz * f1[r].v[e];
-            } else if (act1) {
-                const Coef<T> k1 = coef_at(p, p1);
-                // centre plane t-1 sits in the ring slot requested just before the current one
-                const int slotc = (nwait - 1 + p.nin) % p.nin;
-                const T* pc = IN + (size_t)slotc * in_plane + (wy * R + 1) * TC + cx0;
-                const ZVec<T> sbot = zld(pc - TC);
-                const ZVec<T> ntop = zld(pc + R * TC);
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    T cw = zshfl_up(cc0[r].v[V - 1]);
-                    T ce = zshfl_dn(cc0[r].v[0]);
-                    if (lane == 0) cw = pc[r * TC - 1];
-                    if (lane == 31) ce = pc[r * TC + V];
-                    ZVec<T> o, res;
-                    const ZVec<T>& nn = r == R - 1 ? ntop : cc0[r + 1 < R ? r + 1 : r];
-                    const ZVec<T>& ss = r == 0 ? sbot : cc0[r > 0 ? r - 1 : 0];
-                    if constexpr (sizeof(T) == 8) {
-                        jacobi_vec_d<HAS_RHS>(k1, cc0[r], cw, ce, nn, ss, cp0[r], cm0[r], f1[r], o);
-                    } else {
-                        jacobi_vec_f<HAS_RHS>(k1, p.cz, p.a2, cc0[r], cw, ce, nn, ss, cp0[r], cm0[r], f1[r], o, res);
-                    }
-#pragma unroll
-                    for (int e = 0; e < V; ++e) {
-                        const bool wall = rowwall[r] || colwall[e];
-                        if (NORM && !wall && row_out[r] && col_out && p1 >= kb && p1 < ke) {
-                            double rr;
-                            if constexpr (sizeof(T) == 8) rr = (o.v[e] - cc0[r].v[e]) * k1.iw;
-                            else rr = (double)res.v[e];
-                            acc += rr * rr;
-                        }
-                        u1[r].v[e] = wall ? cc0[r].v[e] : o.v[e];
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int r = 0; r < R; ++r) u1[r] = cc0[r];
-            }
-
-            if (S == 1) {
-                if (p1 >= kb && p1 < ke && col_out) {
-#pragma unroll
-                    for (int r = 0; r < R; ++r)
-                        if (row_out[r]) zst(out + own + p.sp * p1 + (long long)r * p.sx, u1[r]);
-                }
-            }
-
-            // ---------------- stage 2: sweep-2 values of plane t-2 ----------------
-            if (S == 2) {
-                const int p2 = t - 2;
-                if (p2 >= kstart && p2 <= kend_in) {
-                    const Coef<T> k2 = coef_at(p, p2);
-                    const T* pe = EX + (wy * R) * TC + cx0;             // exchange tile holds sweep-1 plane t-2
-                    const ZVec<T> sbot = zld(pe - TC);
-                    const ZVec<T> ntop = zld(pe + R * TC);
-                    const bool st = p2 >= kb && p2 < ke && col_out;
-#pragma unroll
-                    for (int r = 0; r < R; ++r) {
-                        T cw = zshfl_up(cc1[r].v[V - 1]);
-                        T ce = zshfl_dn(cc1[r].v[0]);
-                        if (lane == 0) cw = pe[r * TC - 1];
-                        if (lane == 31) ce = pe[r * TC + V];
-                        ZVec<T> o, res;
-                        const ZVec<T>& nn = r == R - 1 ? ntop : cc1[r + 1 < R ? r + 1 : r];
-                        const ZVec<T>& ss = r == 0 ? sbot : cc1[r > 0 ? r - 1 : 0];
-                        if constexpr (sizeof(T) == 8) {
-                            jacobi_vec_d<HAS_RHS>(k2, cc1[r], cw, ce, nn, ss, u1[r], cm1[r], fprev[r], o);
-                        } else {
-                            jacobi_vec_f<HAS_RHS>(k2, p.cz, p.a2, cc1[r], cw, ce, nn, ss, u1[r], cm1[r], fprev[r], o, res);
-                        }
-#pragma unroll
-                        for (int e = 0; e < V; ++e)
-                            if (rowwall[r] || colwall[e]) o.v[e] = cc1[r].v[e];
-                        if (st && row_out[r]) zst(out + own + p.sp * p2 + (long long)r * p.sx, o);
-                    }
-                }
-            }
-
-            __syncthreads();   // every read of the ring slot of plane t-1 and of the exchange tile is done
-            if (!ZERO) {
-                if (t <= kend_in) ++nwait;
-                // the slot of plane t-1 is free: request the next plane into it
-                if (t > kstart && knext <= kend_in) {
-                    if (warp == 0) issue(knext);
-                    ++nload; ++knext;
-                }
-            }
-            if (S == 2) {
-                T* pe = EX + (wy * R) * TC + cx0;
-#pragma unroll
-                for (int r = 0; r < R; ++r) zst(pe + r * TC, u1[r]);
-                __syncthreads();   // sweep-1 plane t-1 is visible
-#pragma unroll
-                for (int r = 0; r < R; ++r) { cm1[r] = cc1[r]; cc1[r] = u1[r]; fprev[r] = f1[r]; }
-            }
-            if (!ZERO) {
-#pragma unroll
-                for (int r = 0; r < R; ++r) { cm0[r] = cc0[r]; cc0[r] = cp0[r]; }
-            }
+        int t = z.kstart;
+        const int tend = z.ke - 1 + S;
+        z_first<T, ZERO>(p, z, IN, X, t);
+        ++t;
+        while (true) {
+            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, IN, Y, X, Q, P, t);
+            if (++t > tend) break;
+            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, IN, X, Y, P, Q, t);
+            if (++t > tend) break;
         }
-        // drain: planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
+        // planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
     }
     if (NORM) {
         __shared__ double s_red[16];
-        acc = warp_sum(acc);
-        if (lane == 0) s_red[warp] = acc;
+        double a = warp_sum(z.acc);
+        if (lane == 0) s_red[warp] = a;
         __syncthreads();
         if (threadIdx.x == 0) {
             double v = 0.0;
@@ -392,7 +477,7 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
 // ------------------------------------------------------------------------------------------------
 struct ZCfg {
     bool ok = false;
-    int WX = 0, WY = 4, TC = 0, COUT = 0, ntx = 1, ROUT = 0, nty = 0, nin = 4, ctas = 0;
+    int WX = 0, WY = 4, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
     size_t smem = 0;
 };
 
@@ -400,13 +485,15 @@ template <typename T>
 static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
 {
     constexpr int V = ZV<T>::N;
-    constexpr int R = 4;
+    constexpr int NCO = ZV<T>::NCO;
     ZCfg z;
-    if (lv.dim != 3 || lv.coarsest || lv.nz < 5 || lv.sy < 32) return z;
+    if (lv.dim != 3 || lv.coarsest || lv.nz < 5) return z;
     const int lane_cols = 32 * V;
     if (lv.sx % lane_cols != 0) return z;
     const int wfull = lv.sx / lane_cols;
     z.WY = 4;
+    const int NR = z.WY * ZR;
+    if (lv.sy < NR + 1) return z;
     if (wfull <= 4) {
         z.WX = wfull; z.ntx = 1; z.TC = lv.sx; z.COUT = lv.sx;
     } else {
@@ -420,17 +507,19 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
         }
         z.WX = best; z.TC = best * lane_cols; z.COUT = z.TC - 2 * V; z.ntx = (lv.sx + z.COUT - 1) / z.COUT;
     }
-    z.ROUT = z.WY * R - 2 * (S - 1);
-    z.nty = (lv.sy + z.ROUT - 1) / z.ROUT;
-    const size_t in_plane = (size_t)(z.WY * R + 2) * z.TC * sizeof(T);
-    const size_t ex = (size_t)(z.WY * R + 2) * z.TC * sizeof(T);
-    z.nin = 4;
-    while (z.nin > 2 && 128 + (zero ? 0 : z.nin * in_plane) + ex + 256 > 227 * 1024) --z.nin;
-    z.smem = 128 + (zero ? 0 : z.nin * in_plane) + ex + 256;
-    if (z.smem > 227 * 1024) return z;
+    // tiles along y: tile ty has its patch rows at 1 + ty*STEP (the last one is pulled back to end at the wall)
+    z.STEP = NR - 2 * (S - 1);
+    z.nty = lv.sy - NR - 1 <= 0 ? 1 : (lv.sy - NR - 1 + z.STEP - 1) / z.STEP + 1;
     const long long items = (long long)z.ntx * z.nty * (lv.nz - 2);
     // one CTA per SM; a z-segment should be long against its S warm-up planes
     z.ctas = (int)std::max<long long>(1, std::min<long long>(c->num_sms, items / 12));
+    z.zcap = (int)std::min<long long>(lv.nz, (items + z.ctas - 1) / z.ctas + 2 * S + 2);
+    z.coef_bytes = (int)(((size_t)z.zcap * NCO * sizeof(T) + 127) / 128 * 128);
+    z.in_plane = (NR + 2) * z.TC;
+    const size_t plane = (size_t)z.in_plane * sizeof(T);
+    const size_t limit = 227 * 1024 - 256;   // the kernel also has a little static shared memory
+    z.smem = 128 + z.coef_bytes + (zero ? 0 : ZNIN * plane) + 2 * plane;
+    if (z.smem > limit) return z;
     z.ok = true;
     return z;
 }
@@ -452,15 +541,18 @@ static int zsweep_launch(mhs_ctx* c, const Level& lv, const ZCfg& z, const void*
     p.tab = (const T*)lv.tab;
     p.cz = (T)(1.0 / (lv.hz * lv.hz));
     p.a2 = (T)(c->alpha * c->alpha);
-    p.WX = z.WX; p.WY = z.WY; p.TC = z.TC; p.COUT = z.COUT; p.ntx = z.ntx; p.ROUT = z.ROUT; p.nty = z.nty;
+    p.rho = (T)((lv.hy * lv.hy) / (lv.hx * lv.hx));
+    p.WX = z.WX; p.WY = z.WY; p.TC = z.TC; p.COUT = z.COUT; p.ntx = z.ntx; p.STEP = z.STEP; p.nty = z.nty;
     p.NP = lv.nz - 2;
     p.items = (long long)z.ntx * z.nty * p.NP;
-    p.nin = z.nin;
+    p.zcap = z.zcap;
+    p.in_plane = z.in_plane;
+    p.coef_bytes = z.coef_bytes;
     kern<<<z.ctas, z.WX * z.WY * 32, z.smem, c->stream>>>(p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (getenv("MHS_DEBUG")) {
         cudaError_t e = cudaPeekAtLastError();
-        fprintf(stderr, "[mhs] k_zsweep<%s,S=%d,rhs=%d,zero=%d,norm=%d> %dx%dx%d WX %d WY %d TC %d ntx %d nty %d nin %d ctas %d smem %zu: %s\n",
-                sizeof(T) == 8 ? "f64" : "f32", S, (int)HAS_RHS, (int)ZERO, (int)NORM, lv.nx, lv.ny, lv.nz, z.WX, z.WY, z.TC, z.ntx, z.nty, z.nin,
+        fprintf(stderr, "[mhs] k_zsweep<%s,S=%d,rhs=%d,zero=%d,norm=%d> %dx%dx%d WX %d WY %d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
+                sizeof(T) == 8 ? "f64" : "f32", S, (int)HAS_RHS, (int)ZERO, (int)NORM, lv.nx, lv.ny, lv.nz, z.WX, z.WY, z.TC, z.ntx, z.nty,
                 z.ctas, z.smem, cudaGetErrorString(e));
     }
     return z.ctas;
