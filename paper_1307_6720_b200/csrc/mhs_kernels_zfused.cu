@@ -171,32 +171,82 @@ __device__ __forceinline__ void jac_row(const ZCoef<float>& k, float, float cz, 
 // S sweeps.  ZERO: the input iterate is identically zero (coarse-grid correction, first pre-sweep):
 // sweep 1 is u = (omega/D) rhs and no input plane is read at all.
 // ------------------------------------------------------------------------------------------------
+// shared-memory access by 32-bit shared-space address (keeps addresses in one register each)
+template <typename T> __device__ __forceinline__ ZVec<T> lds_vec(uint32_t a);
+template <> __device__ __forceinline__ ZVec<double> lds_vec<double>(uint32_t a)
+{
+    ZVec<double> v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.v[0]), "=d"(v.v[1]) : "r"(a));
+    return v;
+}
+template <> __device__ __forceinline__ ZVec<float> lds_vec<float>(uint32_t a)
+{
+    ZVec<float> v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.v[0]), "=f"(v.v[1]), "=f"(v.v[2]), "=f"(v.v[3]) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts_vec(uint32_t a, const ZVec<double>& v)
+{
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.v[0]), "d"(v.v[1]) : "memory");
+}
+__device__ __forceinline__ void sts_vec(uint32_t a, const ZVec<float>& v)
+{
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.v[0]), "f"(v.v[1]), "f"(v.v[2]), "f"(v.v[3]) : "memory");
+}
+template <typename T> __device__ __forceinline__ T lds_one(uint32_t a);
+template <> __device__ __forceinline__ double lds_one<double>(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+template <> __device__ __forceinline__ float lds_one<float>(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void mbar_wait32(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "ZW2_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+        "@P1 bra ZW2_DONE;\n"
+        "bra ZW2_WAIT;\n"
+        "ZW2_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
 template <typename T>
 struct ZCtx {
-    const T* __restrict__ rhs;    // plane 0 of the right-hand side (uniform)
-    T* __restrict__ out;          // plane 0 of the output (uniform)
-    unsigned own;                 // in-plane offset of (patch row 0, element 0)
-    uint32_t bars;                // shared-space address of the mbarriers
-    const T* coef;                // shared: coefficient records, plane kstart first
-    const T* in_own;              // shared: ring slot 0 + offset of the patch
-    T* ex_own;                    // shared: exchange plane 0 + offset of the patch
-    const T* tile_src;            // global: (first tile row, first tile column) of plane 0
-    int kstart, kend_in, kb, ke;
-    int nload, nwait, knext, stepc;
+    const T* f1;                  // global, per thread: (patch row 0, element 0) of the rhs plane sweep 1 reads in this step
+    T* o_last;                    // global, per thread: same node of the plane the last sweep writes in this step
+    uint32_t bars;                // shared-space addresses: mbarriers,
+    uint32_t coef;                //   coefficient record of the plane sweep 1 makes in this step,
+    uint32_t in_own;              //   ring slot 0 + offset of the patch,
+    uint32_t ex_own;              //   exchange plane 0 + offset of the patch
+    int t;                        // the step: input plane t arrives, sweep 1 makes plane t-1, sweep 2 plane t-2
+    int kb, nout;                 // output planes [kb, kb+nout)
+    int kend_in;                  // last input plane of the segment
+    int zoff;                     // ring position of input plane k is zoff + k
     int omask;                    // rows of the patch that are stored (output rows, output columns)
     bool cw0;                     // element 0 of the patch is a wall column
     double acc;
 };
 
+// warp 0: request input plane `k` of the tile into ring slot nload % ZNIN
 template <typename T>
-__device__ __forceinline__ void z_issue(const ZP<T>& p, ZCtx<T>& z, T* IN, int k)
+__device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int nload, int k)
 {
-    // warp 0: request input plane k into ring slot nload % ZNIN
-    const int slot = z.nload & (ZNIN - 1);
+    const int slot = nload & (ZNIN - 1);
     T* dst = IN + (size_t)slot * p.in_plane;
-    const T* src = z.tile_src + p.sp * k;
+    const T* src = tile_src + p.sp * k;
     const uint32_t plane_bytes = (uint32_t)p.in_plane * sizeof(T);
-    uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + slot;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(bars)) + slot;
     const int lane = threadIdx.x & 31;
     if (p.ntx == 1) {
         if (lane == 0) {
@@ -212,88 +262,97 @@ __device__ __forceinline__ void z_issue(const ZP<T>& p, ZCtx<T>& z, T* IN, int k
     }
 }
 
+// Per-plane coefficients of one sweep (warp-uniform, read from the shared table).
+//   fp64 (expanded update):  u' = A u + By (rho (e+w) + (n+s)) + Bz (up+dn) + wz f ;  iw2 = (D/omega)^2 for the norm
+//   fp32 (difference form):  u' = u + wz (f - L u) with cx, cy per plane
+__device__ __forceinline__ void zc_load(ZCoef<double>& k, uint32_t a, bool rhs, bool norm)
+{
+    const ZVec<double> x = lds_vec<double>(a);
+    k.A = x.v[0]; k.By = x.v[1];
+    if (rhs) {
+        const ZVec<double> y = lds_vec<double>(a + 16);
+        k.Bz = y.v[0]; k.wz = y.v[1];
+    } else {
+        k.Bz = lds_one<double>(a + 16); k.wz = 0.0;
+    }
+    k.iw2 = norm ? lds_one<double>(a + 32) : 0.0;
+}
+__device__ __forceinline__ void zc_load(ZCoef<float>& k, uint32_t a, bool, bool)
+{
+    const ZVec<float> x = lds_vec<float>(a);
+    k.cx = x.v[0]; k.cy = x.v[1]; k.wz = x.v[2];
+}
+
 // End of a plane step: the ring slot of plane t-1 and the exchange plane of t-2 have been read by everybody.
 template <typename T, bool ZERO>
-__device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, T* IN, int t, bool fresh)
+__device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, bool may_issue)
 {
     __syncthreads();
-    if (!ZERO) {
-        if (fresh) ++z.nwait;
-        if (t > z.kstart && z.knext <= z.kend_in) {   // the slot of plane t-1 is free: request the next plane into it
-            if (threadIdx.x < 32) z_issue(p, z, IN, z.knext);
-            ++z.nload;
-            ++z.knext;
-        }
+    if (!ZERO && may_issue) {
+        const int k = z.t + ZNIN - 1;      // the slot of plane t-1 is free: request plane t+ZNIN-1 into it
+        if (k <= z.kend_in && threadIdx.x < 32) z_issue(p, tile_src, z.bars, IN, z.zoff + k, k);
     }
-    ++z.stepc;
+    ++z.t;
 }
 
 // First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
 template <typename T, bool ZERO>
-__device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, T* IN, Patch<T>& dn0, int t)
+__device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0)
 {
     if (!ZERO) {
-        const T* newp = z.in_own + (size_t)(z.nwait & (ZNIN - 1)) * p.in_plane;
-        uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + (z.nwait & (ZNIN - 1));
-        mbar_wait(bar, (uint32_t)((z.nwait / ZNIN) & 1));
+        const int pos = z.zoff + z.t;
+        mbar_wait32(z.bars + 8 * (pos & (ZNIN - 1)), (uint32_t)((pos >> 2) & 1));
+        const uint32_t a = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * (uint32_t)(p.in_plane * sizeof(T));
 #pragma unroll
-        for (int r = 0; r < ZR; ++r) dn0.r[r] = zld(newp + r * p.TC);
+        for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(p.TC * sizeof(T)));
     }
-    z_advance<T, ZERO>(p, z, IN, t, true);
+    z_advance<T, ZERO>(p, z, tile_src, IN, false);
 }
 
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (the step is unrolled twice), so no register is ever moved.
 template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
-__device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1, const Patch<T>& c1,
-                                       int t)
+__device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
+                                       const Patch<T>& c1)
 {
     constexpr int V = ZV<T>::N;
-    constexpr int NCO = ZV<T>::NCO;
-    const int TC = p.TC;
-    const int p1 = t - 1, p2 = t - 2;                  // p1 >= kstart >= 0; p2 >= -1
-    const bool in1 = p1 >= z.kb && p1 < z.ke;          // plane p1 is an output plane of this segment
-    const bool in2 = p2 >= z.kb && p2 < z.ke;
-    const bool fresh = !ZERO && t <= z.kend_in;        // a new input plane arrives in this step
+    constexpr uint32_t ES = sizeof(T);
+    const uint32_t rowb = (uint32_t)p.TC * ES;
+    const uint32_t planeb = (uint32_t)p.in_plane * ES;
+    const int t = z.t;
+    const bool in1 = (unsigned)(t - 1 - z.kb) < (unsigned)z.nout;   // plane t-1 is an output plane of this segment
+    const bool in2 = (unsigned)(t - 2 - z.kb) < (unsigned)z.nout;
+    const bool fresh = !ZERO && t <= z.kend_in;                      // a new input plane arrives in this step
+    const int pos = z.zoff + t;
     // !fresh (only the step after the top plane): the slot holds an older plane -- finite numbers that meet Bz = 0
-    const T* newp = z.in_own + (size_t)(z.nwait & (ZNIN - 1)) * p.in_plane;          // plane t
-    const T* cenp = z.in_own + (size_t)((z.nwait - 1) & (ZNIN - 1)) * p.in_plane;    // plane t-1
-    T* exw = z.ex_own + (size_t)(z.stepc & 1) * p.in_plane;                            // sweep-1 plane t-1 (written now)
-    const T* exr = z.ex_own + (size_t)((z.stepc & 1) ^ 1) * p.in_plane;                // sweep-1 plane t-2 (written a step ago)
-    if (fresh) {
-        uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + (z.nwait & (ZNIN - 1));
-        mbar_wait(bar, (uint32_t)((z.nwait / ZNIN) & 1));
-    }
+    const uint32_t a_new = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * planeb;          // plane t
+    const uint32_t a_cen = z.in_own + (uint32_t)((pos - 1) & (ZNIN - 1)) * planeb;    // plane t-1
+    const uint32_t a_exw = z.ex_own + (uint32_t)(t & 1) * planeb;                      // sweep-1 plane t-1 (written now)
+    const uint32_t a_exr = z.ex_own + (uint32_t)((t & 1) ^ 1) * planeb;                // sweep-1 plane t-2 (written a step ago)
+    if (fresh) mbar_wait32(z.bars + 8 * (pos & (ZNIN - 1)), (uint32_t)((pos >> 2) & 1));
     ZCoef<T> k1, k2;
-    k1.load(z.coef + (p1 - z.kstart) * NCO, HAS_RHS, NORM);
-    if (S == 2) k2.load(z.coef + max(p2 - z.kstart, 0) * NCO, HAS_RHS, false);
-    // uniform plane bases + 32-bit per-thread offsets
-    const T* f1p = HAS_RHS ? z.rhs + p.sp * p1 : nullptr;
-    const T* f2p = HAS_RHS ? z.rhs + p.sp * max(p2, 0) : nullptr;
-    T* o1p = z.out + p.sp * p1;
-    T* o2p = z.out + p.sp * max(p2, 0);
+    zc_load(k1, z.coef, HAS_RHS, NORM);
+    if (S == 2) zc_load(k2, z.coef - ZV<T>::NCO * ES, HAS_RHS, false);
     const int m1 = in1 ? z.omask : 0, m2 = in2 ? z.omask : 0;
-    ZVec<T> s1, n1, s2, n2;
-    if (!ZERO) { s1 = zld(cenp - TC); n1 = zld(cenp + ZR * TC); }
-    if (S == 2) { s2 = zld(exr - TC); n2 = zld(exr + ZR * TC); }
     double pa = 0.0;
     float pf = 0.f;
 #pragma unroll
     for (int r = 0; r < ZR; ++r) {
-        const unsigned goff = z.own + (unsigned)r * (unsigned)p.sx;
+        const long long grow = (long long)r * p.sx;
         // ---------------- stage 1: sweep-1 values of row r of plane t-1 ----------------
         ZVec<T> up0, o1, f1;
-        if (!ZERO) up0 = zld(newp + r * TC);
-        if (HAS_RHS) f1 = zld(f1p + goff);
+        if (!ZERO) up0 = lds_vec<T>(a_new + r * rowb);
+        if (HAS_RHS) f1 = zld(z.f1 + grow);
         if (ZERO) {
 #pragma unroll
             for (int e = 0; e < V; ++e) o1.v[e] = k1.wz * f1.v[e];
             if (z.cw0) o1.v[0] = T(0);
         } else {
-            const T w = cenp[r * TC - 1], e = cenp[r * TC + V];
-            const ZVec<T>& nn = r == ZR - 1 ? n1 : c0.r[r + 1 < ZR ? r + 1 : r];
-            const ZVec<T>& ss = r == 0 ? s1 : c0.r[r > 0 ? r - 1 : 0];
+            const T w = lds_one<T>(a_cen + r * rowb - ES), e = lds_one<T>(a_cen + r * rowb + V * ES);
+            ZVec<T> nn, ss;
+            if (r == ZR - 1) nn = lds_vec<T>(a_cen + ZR * rowb); else nn = c0.r[r + 1 < ZR ? r + 1 : r];
+            if (r == 0) ss = lds_vec<T>(a_cen - rowb); else ss = c0.r[r > 0 ? r - 1 : 0];
             float rs = 0.f;
             jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], w, e, nn, ss, up0, dn0.r[r], f1, o1, z.cw0, rs);
             if (z.cw0) o1.v[0] = c0.r[r].v[0];
@@ -311,27 +370,31 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, T* IN, Patch<
             dn0.r[r] = up0;     // becomes the centre plane of the next step
         }
         if (S == 1) {
-            if (m1 & (1 << r)) zst(o1p + goff, o1);
+            if (m1 & (1 << r)) zst(z.o_last + grow, o1);
         } else {
-            zst(exw + r * TC, o1);
+            sts_vec(a_exw + r * rowb, o1);
             // ---------------- stage 2: sweep-2 values of row r of plane t-2 ----------------
             ZVec<T> o2, f2;
-            if (HAS_RHS) f2 = zld(f2p + goff);
-            const T w = exr[r * TC - 1], e = exr[r * TC + V];
-            const ZVec<T>& nn = r == ZR - 1 ? n2 : c1.r[r + 1 < ZR ? r + 1 : r];
-            const ZVec<T>& ss = r == 0 ? s2 : c1.r[r > 0 ? r - 1 : 0];
+            if (HAS_RHS) f2 = zld(z.f1 - p.sp + grow);
+            const T w = lds_one<T>(a_exr + r * rowb - ES), e = lds_one<T>(a_exr + r * rowb + V * ES);
+            ZVec<T> nn, ss;
+            if (r == ZR - 1) nn = lds_vec<T>(a_exr + ZR * rowb); else nn = c1.r[r + 1 < ZR ? r + 1 : r];
+            if (r == 0) ss = lds_vec<T>(a_exr - rowb); else ss = c1.r[r > 0 ? r - 1 : 0];
             float rs;
             jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], w, e, nn, ss, o1, dn1.r[r], f2, o2, false, rs);
             if (z.cw0) o2.v[0] = c1.r[r].v[0];
-            if (m2 & (1 << r)) zst(o2p + goff, o2);
+            if (m2 & (1 << r)) zst(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
         }
     }
     if (NORM) {
-        if (sizeof(T) == 8) z.acc = fma(zc_iw2(k1), pa, z.acc);   // pa == 0 unless plane p1 is an output plane
+        if (sizeof(T) == 8) z.acc = fma(zc_iw2(k1), pa, z.acc);   // pa == 0 unless plane t-1 is an output plane
         else z.acc += (double)pf;
     }
-    z_advance<T, ZERO>(p, z, IN, t, fresh);
+    z.coef += ZV<T>::NCO * ES;
+    z.o_last += p.sp;
+    if (HAS_RHS) z.f1 += p.sp;
+    z_advance<T, ZERO>(p, z, tile_src, IN, true);
 }
 
 template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
@@ -349,9 +412,9 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
     const int wx = warp % p.WX, wy = warp / p.WX;
     const int TC = p.TC;
     const int NR = p.WY * ZR;                              // patch rows of a tile
-    // shared memory: [mbarriers: 128 B] [coefficients] [IN ring: ZNIN planes] [EX: 2 exchange planes]
+    // shared memory: [mbarriers: 128 B] [coefficients: a pad record + zcap records] [IN ring: ZNIN planes] [EX: 2 planes]
     uint64_t* bars = reinterpret_cast<uint64_t*>(zsm);
-    T* coef = reinterpret_cast<T*>(zsm + 128);
+    T* coef = reinterpret_cast<T*>(zsm + 128) + NCO;       // record of plane kstart; the record before it is a pad
     T* IN = reinterpret_cast<T*>(zsm + 128 + p.coef_bytes);
     T* EX = IN + (size_t)(ZERO ? 0 : ZNIN) * p.in_plane;
 
@@ -362,27 +425,23 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
     if (S == 2) {   // guard rows and never-written parts of the exchange planes must hold zeros (a wall row may sit there)
         for (int q = threadIdx.x; q < 2 * p.in_plane; q += blockDim.x) EX[q] = T(0);
     }
+    if (threadIdx.x < NCO) coef[-NCO + (int)threadIdx.x] = T(0);
     __syncthreads();
 
     const int cx0 = (wx * 32 + lane) * V;                   // first column of this thread's vector inside the tile
     ZCtx<T> z;
-    z.rhs = rhs;
-    z.out = out;
     z.bars = smem_u32(bars);
-    z.coef = coef;
-    z.in_own = IN + (wy * ZR + 1) * TC + cx0;
-    z.ex_own = EX + (wy * ZR + 1) * TC + cx0;
-    z.nload = 0;                                            // planes requested so far by this CTA (ring position)
-    z.nwait = 0;                                            // planes consumed so far
-    z.stepc = 0;
+    z.in_own = smem_u32(IN + (wy * ZR + 1) * TC + cx0);
+    z.ex_own = smem_u32(EX + (wy * ZR + 1) * TC + cx0);
     z.acc = 0.0;
+    int ring = 0;                                           // planes requested so far by this CTA (ring position)
     const long long q0 = p.items * blockIdx.x / gridDim.x, q1 = p.items * (blockIdx.x + 1) / gridDim.x;
 
     for (long long q = q0; q < q1;) {
         const int tile = (int)(q / p.NP);
-        z.kb = 1 + (int)(q - (long long)tile * p.NP);
-        z.ke = (int)min((long long)p.NP + 1, z.kb + (q1 - q));   // output planes [kb, ke)
-        q += z.ke - z.kb;
+        const int kb = 1 + (int)(q - (long long)tile * p.NP);
+        const int ke = (int)min((long long)p.NP + 1, kb + (q1 - q));   // output planes [kb, ke)
+        q += ke - kb;
         const int ty = tile / p.ntx, tx = tile - ty * p.ntx;
         const int ct = p.ntx == 1 ? 0 : tx * p.COUT - V;              // first column of the tile
         // Tiles along y: patch rows [jt, jt+NR) are interior rows; the wall rows j = 0 / j = sy are only ever
@@ -390,14 +449,14 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
         const int jt = min(1 + ty * p.STEP, p.sy - NR);                // first patch row
         const int jlo = ty == 0 ? 1 : 1 + ty * p.STEP + H;             // rows [jlo, jhi) are this tile's output
         const int jhi = ty == p.nty - 1 ? p.sy : 1 + ty * p.STEP + NR - H;
-        z.kstart = max(z.kb - S, 0);
-        z.kend_in = min(z.ke - 1 + S, p.nz - 1);
-        z.tile_src = u + (long long)(jt - 1) * p.sx + ct;             // (row jt-1, col ct) of plane 0
+        const int kstart = max(kb - S, 0);
+        const int kend_in = min(ke - 1 + S, p.nz - 1);
+        const T* tile_src = u + (long long)(jt - 1) * p.sx + ct;      // (row jt-1, col ct) of plane 0
 
         // per-plane coefficient records of this segment
         __syncthreads();   // the previous segment is done with the table
-        for (int i = threadIdx.x; i < (z.kend_in - z.kstart + 1) * NCO; i += blockDim.x) {
-            const int k = z.kstart + i / NCO, c = i % NCO;
+        for (int i = threadIdx.x; i < (kend_in - kstart + 1) * NCO; i += blockDim.x) {
+            const int k = kstart + i / NCO, c = i % NCO;
             const T* t = p.tab;
             T v = T(0);
             if (sizeof(T) == 8) {
@@ -414,15 +473,12 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
             }
             coef[i] = v;
         }
-
-        z.knext = z.kstart;     // next plane to request
+        z.zoff = ring - kstart;
         if (!ZERO) {
-            const int n = min(ZNIN, z.kend_in - z.knext + 1);
-            for (int i = 0; i < n; ++i) {
-                if (warp == 0) z_issue(p, z, IN, z.knext + i);
-                ++z.nload;
-            }
-            z.knext += n;
+            const int n = min(ZNIN, kend_in - kstart + 1);
+            if (warp == 0)
+                for (int i = 0; i < n; ++i) z_issue(p, tile_src, z.bars, IN, ring + i, kstart + i);
+            ring += kend_in - kstart + 1;
         }
         __syncthreads();   // coefficient table visible
 
@@ -437,9 +493,16 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
             const int j = jrow0 + r;
             if (col_out && j >= jlo && j < jhi) z.omask |= 1 << r;
         }
-        // in-plane offset of (patch row 0, element 0).  jrow0 >= 1; icol0 >= -V only for halo vectors of the first
-        // x tile, which neither load nor store through it: clamp
-        z.own = (unsigned)(jrow0 * p.sx + max(icol0, 0));
+        // in-plane offset of (patch row 0, element 0); halo vectors left of column 0 neither load nor store through it
+        const long long own = (long long)jrow0 * p.sx + max(icol0, 0);
+        z.t = kstart;
+        z.kb = kb;
+        z.nout = ke - kb;
+        z.kend_in = kend_in;
+        z.coef = smem_u32(coef);
+        // the first z_step runs at t = kstart+1: sweep 1 makes plane kstart, sweep 2 plane kstart-1
+        z.f1 = rhs + own + p.sp * kstart;
+        z.o_last = out + own + p.sp * (kstart - (S - 1));
 
         Patch<T> X, Y, P, Q;
 #pragma unroll
@@ -447,15 +510,13 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
 #pragma unroll
             for (int e = 0; e < V; ++e) X.r[r].v[e] = Y.r[r].v[e] = P.r[r].v[e] = Q.r[r].v[e] = T(0);
 
-        int t = z.kstart;
-        const int tend = z.ke - 1 + S;
-        z_first<T, ZERO>(p, z, IN, X, t);
-        ++t;
+        const int tend = ke - 1 + S;
+        z_first<T, ZERO>(p, z, tile_src, IN, X);
         while (true) {
-            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, IN, Y, X, Q, P, t);
-            if (++t > tend) break;
-            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, IN, X, Y, P, Q, t);
-            if (++t > tend) break;
+            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, Y, X, Q, P);
+            if (z.t > tend) break;
+            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, X, Y, P, Q);
+            if (z.t > tend) break;
         }
         // planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
     }
@@ -514,7 +575,7 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
     // one CTA per SM; a z-segment should be long against its S warm-up planes
     z.ctas = (int)std::max<long long>(1, std::min<long long>(c->num_sms, items / 12));
     z.zcap = (int)std::min<long long>(lv.nz, (items + z.ctas - 1) / z.ctas + 2 * S + 2);
-    z.coef_bytes = (int)(((size_t)z.zcap * NCO * sizeof(T) + 127) / 128 * 128);
+    z.coef_bytes = (int)(((size_t)(z.zcap + 1) * NCO * sizeof(T) + 127) / 128 * 128);
     z.in_plane = (NR + 2) * z.TC;
     const size_t plane = (size_t)z.in_plane * sizeof(T);
     const size_t limit = 227 * 1024 - 256;   // the kernel also has a little static shared memory
