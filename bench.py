@@ -41,6 +41,34 @@ def peaks():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def reduce_over_ranks(ms, cycles, world, device="cuda"):
+    """(max over ranks of the device time, sum over ranks of the cycles done): the only cross-rank
+    traffic of a replica run.  `device="cpu"` serves the gloo test (tests/test_replicas_gloo.py)."""
+    if world <= 1:
+        return ms, cycles
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor([cycles], device=device, dtype=torch.float64)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(c.item())
+
+
+def read_traffic(key):
+    """profiles/traffic.csv: `key,value` rows copied from the committed `ncu --set full` capture
+    (dram__bytes_read.sum + dram__bytes_write.sum per launch of the named kernel); None if absent."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for line in open(p):
+            k, _, v = line.strip().partition(",")
+            if k == key:
+                return float(v)
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -199,15 +227,7 @@ def main():
         e1.record()
         barrier()
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-            cc = torch.tensor([c3], device="cuda", dtype=torch.float64)
-            dist.all_reduce(cc, op=dist.ReduceOp.SUM)
-            c3_all = int(cc.item())
-        else:
-            c3_all = c3
+        ms, c3_all = reduce_over_ranks(ms, c3, world)
         return ms, c2, c3, c3_all, last
 
     for _ in range(max(args.warmup, 0)):
@@ -233,13 +253,7 @@ def main():
     # (2w/s per update, s sweeps per launch) -> 2*w*n_int per launch
     bytes_per_launch = 2.0 * es * n_int
     achieved = bytes_per_launch * launches / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get("smooth_l0_dram_bytes_per_launch_%d" % w.nx)
-        except Exception:
-            traffic = None
+    traffic = read_traffic("smooth_l0_dram_bytes_per_launch_%d" % w.nx)
     roof = {"bound": "hbm", "kernel": "finest-level weighted-Jacobi smoother (kernel class smooth_l0)",
             "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
             "frac_of_8TBs_nominal": achieved / 8000.0, "traffic": traffic,
