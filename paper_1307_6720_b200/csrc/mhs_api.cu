@@ -257,7 +257,7 @@ bool use_fast(const mhs_ctx* ctx, const Level& lv)
 
 bool use_zsweep(const mhs_ctx* ctx, const Level& lv)
 {
-    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && zsweep_ok(ctx, lv);
+    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && !mid_level(lv) && zsweep_ok(ctx, lv);
 }
 
 int clus_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->clus3 : ctx->clus2; }
@@ -341,6 +341,11 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
             const int S = std::min(2, n_pre);
             launch_zsweep(ctx, lv, nullptr, rhs, lv.u, S, true, false, done);
             n_pre -= S;
+        } else if (fast && n_pre >= 2) {
+            // the first two sweeps from zero in one pass over rhs (sweep 1, u = (omega/D) rhs, is never stored)
+            launch_smooth_z(ctx, lv, nullptr, rhs, lv.u, 3, ctx->dir, done);
+            ctx->dir ^= 1;
+            n_pre -= 2;
         } else if (fast && n_pre >= 1) {
             launch_scale_rhs(ctx, lv, rhs, lv.u, done);  // first sweep from zero: u = (omega/D) rhs
             n_pre -= 1;

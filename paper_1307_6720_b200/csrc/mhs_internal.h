@@ -109,7 +109,9 @@ void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void
 
 // ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);
-// mode 0: sweep; 1: sweep + partial sums of the INPUT's ||rhs - L u||^2; 2: partial sums only.  Returns #partials.
+bool mid_level(const Level& lv);   // small enough to live in the L2: parallelism-bound, gets fine-grained launch shapes
+// mode 0: sweep; 1: sweep + partial sums of the INPUT's ||rhs - L u||^2; 2: partial sums only; 3: the first two sweeps
+// from the zero initial guess in one pass (u not read).  Returns #partials.
 long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done);
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);

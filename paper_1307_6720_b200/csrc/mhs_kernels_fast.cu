@@ -59,12 +59,18 @@ __device__ __forceinline__ void residual_vec(const Vec<T>& c, T cw, T ce, const 
 //   STORE : write out = u + (omega/D_k) r          NORM : accumulate sum r^2 into partial[block]
 // Work item q <-> (row group g, x vector xv): rows j0 = g*R .. j0+R-1, elements i0 = xv*V .. i0+V-1.
 // ------------------------------------------------------------------------------------------------
-template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM>
+//   ZERO2 : the iterate is the result of the first sweep from the zero initial guess of a coarse-grid correction,
+//           u1 = (omega/D_k) rhs (0 on the planes k = 0, nz-1 and on the walls, where rhs is 0); it is never stored:
+//           `u` is not read, its values are formed from rhs on the fly, so "two sweeps from zero" is ONE pass that
+//           reads rhs and writes u2.
+template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM, bool ZERO2>
 __global__ void __launch_bounds__(128) k_smooth_z(LP<T> p, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ out,
                                                    int kchunk, int nzc, int reverse, double* __restrict__ partial,
                                                    const int* __restrict__ done)
 {
+    static_assert(!ZERO2 || (HAS_RHS && STORE && !NORM), "ZERO2 is a plain sweep with a right-hand side");
     if (done && *done) return;
+    if (ZERO2) u = rhs;
     constexpr int V = VN<T>::N;
     const int nvx = p.sx / V;
     const int ngroups = (p.sy + R - 1) / R;
@@ -82,26 +88,41 @@ __global__ void __launch_bounds__(128) k_smooth_z(LP<T> p, const T* __restrict__
     const long long base = i0 + (long long)p.sx * j0;
     const T* tab = p.tab;
 
+    const T* wz = tab + 9 * (long long)p.nz;   // omega/D_k on interior planes, 0 on k = 0 and k = nz-1
     Vec<T> cm[R], cc[R], cp[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         cm[r] = ldv(u + base + (long long)p.sx * r + p.sp * (kb - 1));
         cc[r] = ldv(u + base + (long long)p.sx * r + p.sp * kb);
+        if (ZERO2) {
+            const T a = wz[kb - 1], b = wz[kb];
+#pragma unroll
+            for (int e = 0; e < V; ++e) { cm[r].v[e] *= a; cc[r].v[e] *= b; }
+        }
     }
     double acc = 0.0;
     for (int k = kb; k < ke; ++k) {
         const T* pl = u + base + p.sp * k;
 #pragma unroll
         for (int r = 0; r < R; ++r) cp[r] = ldv(pl + p.sp + (long long)p.sx * r);
-        const Vec<T> ntop = ldv(pl + (long long)p.sx * R);
-        const Vec<T> sbot = ldv(pl - p.sx);
+        Vec<T> ntop = ldv(pl + (long long)p.sx * R);
+        Vec<T> sbot = ldv(pl - p.sx);
         const T cx = tab[k], cy = tab[p.nz + k], wk = tab[3 * p.nz + k];
+        if (ZERO2) {
+            const T a = wz[k + 1];
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+#pragma unroll
+                for (int e = 0; e < V; ++e) cp[r].v[e] *= a;
+#pragma unroll
+            for (int e = 0; e < V; ++e) { ntop.v[e] *= wk; sbot.v[e] *= wk; }
+        }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             T cw = shfl_up1(cc[r].v[V - 1]);
             T ce = shfl_dn1(cc[r].v[0]);
-            if (lane == 0) cw = pl[(long long)p.sx * r - 1];
-            if (lane == 31) ce = pl[(long long)p.sx * r + V];
+            if (lane == 0) cw = ZERO2 ? wk * pl[(long long)p.sx * r - 1] : pl[(long long)p.sx * r - 1];
+            if (lane == 31) ce = ZERO2 ? wk * pl[(long long)p.sx * r + V] : pl[(long long)p.sx * r + V];
             Vec<T> f, res;
             if (HAS_RHS) f = ldv(rhs + base + p.sp * k + (long long)p.sx * r);
             residual_vec<T>(cc[r], cw, ce, r == R - 1 ? ntop : cc[r + 1 < R ? r + 1 : r], r == 0 ? sbot : cc[r > 0 ? r - 1 : 0],
@@ -320,11 +341,15 @@ static int pick_chunks(long long xy_blocks, int planes, int slots, int min_chunk
     return best;
 }
 
-template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM>
+// Levels that fit in the L2 several times over (<= ~5 M nodes: 129^3 and below) are not bandwidth problems but
+// parallelism problems: they get one row per thread and short z-chunks, so that even 65^3 fills the 148 SMs.
+bool mid_level(const Level& lv) { return lv.npts() <= 5000000LL; }
+
+template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM, bool ZERO2>
 static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int reverse, const int* done)
 {
     constexpr int V = VN<T>::N;
-    auto kern = k_smooth_z<T, R, HAS_RHS, STORE, NORM>;
+    auto kern = k_smooth_z<T, R, HAS_RHS, STORE, NORM, ZERO2>;
     static int slots = 0;
     if (!slots) {
         int nb = 0;
@@ -334,7 +359,7 @@ static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const vo
     const long long items = (long long)((lv.sy + R - 1) / R) * (lv.sx / V);
     const long long xb = (items + 127) / 128;
     const int planes = lv.nz - 2;
-    const int nzc = pick_chunks(xb, planes, slots, 8);
+    const int nzc = pick_chunks(xb, planes, slots, R == 1 ? 2 : 8);
     const int kchunk = (planes + nzc - 1) / nzc;
     const int nzc2 = (planes + kchunk - 1) / kchunk;
     dim3 grid((unsigned)xb, (unsigned)nzc2);
@@ -342,24 +367,27 @@ static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const vo
     return xb * nzc2;
 }
 
-// mode: 0 = sweep, 1 = sweep + norm of the input residual, 2 = norm only.  Returns the number of partials.
+// mode: 0 = sweep, 1 = sweep + norm of the input residual, 2 = norm only, 3 = the first TWO sweeps from the zero
+// initial guess (u is not read).  Returns the number of partials.
 long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done)
 {
     count_launch(c);
-#define SZ(T, R)                                                                                              \
-    do {                                                                                                      \
-        if (rhs) {                                                                                            \
-            if (mode == 0) return smooth_z_t<T, R, true, true, false>(c, lv, u, rhs, out, reverse, done);     \
-            if (mode == 1) return smooth_z_t<T, R, true, true, true>(c, lv, u, rhs, out, reverse, done);      \
-            return smooth_z_t<T, R, true, false, true>(c, lv, u, rhs, out, reverse, done);                    \
-        } else {                                                                                              \
-            if (mode == 0) return smooth_z_t<T, R, false, true, false>(c, lv, u, rhs, out, reverse, done);    \
-            if (mode == 1) return smooth_z_t<T, R, false, true, true>(c, lv, u, rhs, out, reverse, done);     \
-            return smooth_z_t<T, R, false, false, true>(c, lv, u, rhs, out, reverse, done);                   \
-        }                                                                                                     \
+#define SZ(T, R)                                                                                                     \
+    do {                                                                                                             \
+        if (mode == 3) return smooth_z_t<T, R, true, true, false, true>(c, lv, u, rhs, out, reverse, done);          \
+        if (rhs) {                                                                                                   \
+            if (mode == 0) return smooth_z_t<T, R, true, true, false, false>(c, lv, u, rhs, out, reverse, done);     \
+            if (mode == 1) return smooth_z_t<T, R, true, true, true, false>(c, lv, u, rhs, out, reverse, done);      \
+            return smooth_z_t<T, R, true, false, true, false>(c, lv, u, rhs, out, reverse, done);                    \
+        } else {                                                                                                     \
+            if (mode == 0) return smooth_z_t<T, R, false, true, false, false>(c, lv, u, rhs, out, reverse, done);    \
+            if (mode == 1) return smooth_z_t<T, R, false, true, true, false>(c, lv, u, rhs, out, reverse, done);     \
+            return smooth_z_t<T, R, false, false, true, false>(c, lv, u, rhs, out, reverse, done);                   \
+        }                                                                                                            \
     } while (0)
-    if (c->es == 8) SZ(double, 4);
-    else SZ(float, 4);
+    const bool mid = mid_level(lv);
+    if (c->es == 8) { if (mid) SZ(double, 1); SZ(double, 4); }
+    else { if (mid) SZ(float, 1); SZ(float, 4); }
 #undef SZ
     return 0;
 }
@@ -367,8 +395,9 @@ long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
 {
     const int V = c->es == 8 ? 2 : 4;
-    const long long items = (long long)((lv.sy + 3) / 4) * (lv.sx / V);
-    return ((items + 127) / 128) * (long long)std::max(1, (lv.nz - 2 + 7) / 8 + 1);
+    const int R = mid_level(lv) ? 1 : 4;
+    const long long items = (long long)((lv.sy + R - 1) / R) * (lv.sx / V);
+    return ((items + 127) / 128) * (long long)std::max(1, (lv.nz - 2 + 1) / 2 + 1);
 }
 
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done)
@@ -380,11 +409,10 @@ void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, con
     else k_scale_rhs<float><<<grid, 256, 0, c->stream>>>(lp_of<float>(c, lv), (const float*)rhs, (float*)u, done);
 }
 
-template <typename T, bool HAS_RHS>
+template <typename T, int R, bool HAS_RHS>
 static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
 {
     constexpr int V = VN<T>::N;
-    constexpr int R = 4;
     auto kern = k_resid_restrict_z<T, R, HAS_RHS>;
     static int slots = 0;
     if (!slots) {
@@ -396,7 +424,7 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
     const long long warps = (items + 1 + 30) / 31;   // lanes 1..31 of each warp carry items
     const long long xb = (warps + 3) / 4;
     const int planes = co.nz - 2;
-    const int nzc = pick_chunks(xb, planes, slots, 4);
+    const int nzc = pick_chunks(xb, planes, slots, R == 2 ? 1 : 4);
     const int Kchunk = (planes + nzc - 1) / nzc;
     const int nzc2 = (planes + Kchunk - 1) / Kchunk;
     dim3 grid((unsigned)xb, (unsigned)nzc2);
@@ -406,13 +434,20 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
 void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
 {
     count_launch(c);
-    if (c->es == 8) {
-        if (rhs) resid_restrict_t<double, true>(c, f, u, rhs, co, rc, reverse, done);
-        else resid_restrict_t<double, false>(c, f, u, rhs, co, rc, reverse, done);
-    } else {
-        if (rhs) resid_restrict_t<float, true>(c, f, u, rhs, co, rc, reverse, done);
-        else resid_restrict_t<float, false>(c, f, u, rhs, co, rc, reverse, done);
-    }
+    const bool mid = mid_level(f);
+#define RR(T)                                                                                  \
+    do {                                                                                       \
+        if (mid) {                                                                             \
+            if (rhs) resid_restrict_t<T, 2, true>(c, f, u, rhs, co, rc, reverse, done);        \
+            else resid_restrict_t<T, 2, false>(c, f, u, rhs, co, rc, reverse, done);           \
+        } else {                                                                               \
+            if (rhs) resid_restrict_t<T, 4, true>(c, f, u, rhs, co, rc, reverse, done);        \
+            else resid_restrict_t<T, 4, false>(c, f, u, rhs, co, rc, reverse, done);           \
+        }                                                                                      \
+    } while (0)
+    if (c->es == 8) RR(double);
+    else RR(float);
+#undef RR
 }
 
 void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, const void* ec, int reverse, const int* done)
