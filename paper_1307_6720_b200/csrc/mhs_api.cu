@@ -750,7 +750,13 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
     if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
     if (!B && !p && !rho) return MHS_OK;
     Scope sc(ctx, MHS_KC_FIELDS);
-    launch_fields_ref(ctx, ctx->L3[0], ctx->L3[0].u, B, p, rho);
+    const Level& l0 = ctx->L3[0];
+    if (!(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fields_z_ok(ctx, l0)) {
+        launch_fields_z(ctx, l0, l0.u, B, p, rho);
+        launch_fields_ref(ctx, l0, l0.u, B, p, rho, true);
+    } else {
+        launch_fields_ref(ctx, l0, l0.u, B, p, rho);
+    }
     CK(cudaGetLastError());
     return MHS_OK;
 }

@@ -105,7 +105,10 @@ long long resnorm_partial_capacity(const Level& lv);
 void launch_norm_final(mhs_ctx* c, long long n, int mode);
 void launch_pack(mhs_ctx* c, const Level& lv, const void* dense, void* dst, bool keep_bottom, bool negate);
 void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense);
-void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
+void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only = false);
+// ---- one-pass field recovery (mhs_kernels_fields.cu): planes 1 .. nz-2 ----
+bool fields_z_ok(const mhs_ctx* c, const Level& lv);
+void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
 
 // ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);

@@ -212,11 +212,11 @@ __device__ __forceinline__ T Bz_at(const FieldsP<T>& q, const T* P, int i, int j
 
 template <typename T>
 __global__ void __launch_bounds__(256) k_fields_ref(FieldsP<T> q, const T* __restrict__ P, T* __restrict__ Bx, T* __restrict__ By,
-                                                     T* __restrict__ Bz, T* __restrict__ pp, T* __restrict__ rho)
+                                                     T* __restrict__ Bz, T* __restrict__ pp, T* __restrict__ rho, int kstride)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
+    const int k = blockIdx.z * kstride;
     if (i >= q.nx || j >= q.ny) return;
     const long long d = i + (long long)q.nx * (j + (long long)q.ny * k);
     const T xi = q.ft[k], dxi = q.ft[q.nz + k], pb = q.ft[2 * q.nz + k], rb = q.ft[3 * q.nz + k];
@@ -355,7 +355,7 @@ void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense)
 }
 
 template <typename T>
-static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho)
+static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only)
 {
     FieldsP<T> q;
     q.nx = lv.nx; q.ny = lv.ny; q.nz = lv.nz; q.sx = lv.sx; q.sp = lv.sp;
@@ -365,17 +365,19 @@ static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, vo
     q.i2mu0 = (T)(1.0 / (2.0 * c->opt.mu0)); q.imu0 = (T)(1.0 / c->opt.mu0); q.ig = (T)(1.0 / c->opt.g);
     q.ft = (const T*)c->prof_tab;
     const dim3 b(32, 8);
-    const dim3 g((lv.nx + 31) / 32, (lv.ny + 7) / 8, lv.nz);
+    const dim3 g((lv.nx + 31) / 32, (lv.ny + 7) / 8, ends_only ? 2 : lv.nz);
     const long long N = lv.npts();
     T* Bx = (T*)B;
-    k_fields_ref<T><<<g, b, 0, c->stream>>>(q, (const T*)P, Bx, Bx ? Bx + N : nullptr, Bx ? Bx + 2 * N : nullptr, (T*)p, (T*)rho);
+    k_fields_ref<T><<<g, b, 0, c->stream>>>(q, (const T*)P, Bx, Bx ? Bx + N : nullptr, Bx ? Bx + 2 * N : nullptr, (T*)p, (T*)rho,
+                                            ends_only ? lv.nz - 1 : 1);
 }
 
-void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho)
+// ends_only: just the planes k = 0 and k = nz-1 (the rest is done by launch_fields_z)
+void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only)
 {
     count_launch(c);
-    if (c->es == 8) fields_ref_t<double>(c, lv, P, B, p, rho);
-    else fields_ref_t<float>(c, lv, P, B, p, rho);
+    if (c->es == 8) fields_ref_t<double>(c, lv, P, B, p, rho, ends_only);
+    else fields_ref_t<float>(c, lv, P, B, p, rho, ends_only);
 }
 
 }  // namespace mhs

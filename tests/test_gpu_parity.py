@@ -46,6 +46,8 @@ WORKLOADS = {
     "ragged_25x49x13": lambda: inputs.small(nx=25, ny=49, nz=13, L=(1.0, 1.7, 0.6), seed=7),
     "cfg1_65": lambda: inputs.config(1, shrink=2),
     "cfg3_v33_65": lambda: inputs.config(3, shrink=8),
+    "cfg1_129": lambda: inputs.config(1),          # sx = 128: the vector kernels' fp32 shapes (128-column warps)
+    "slab_129x65x33": lambda: inputs.small(nx=129, ny=65, nz=33, L=(2.0, 1.0, 0.5), seed=11),
 }
 VARIANTS = {"fast": 0, "reference": 1}
 
@@ -217,7 +219,7 @@ def test_config0_cycle_counts(B):
 # ------------------------------------------------------------------ fields -------------------
 @pytest.mark.parametrize("variant", list(VARIANTS))
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
-@pytest.mark.parametrize("name", ["cfg0_33", "ragged_17x33x9", "cfg1_65"])
+@pytest.mark.parametrize("name", ["cfg0_33", "ragged_17x33x9", "cfg1_65", "cfg1_129", "slab_129x65x33"])
 def test_fields_parity(B, orc, name, dtype, variant):
     w = WORKLOADS[name]()
     P = inputs.random_field(w.shape, 77) * 1e-2
@@ -328,6 +330,24 @@ def test_odd_sweep_counts_and_v11(B, orc):
             Po, oi = orc.solve_interior(P, w.f, w.alpha, w.L, omega=w.omega, n_pre=a, n_post=b, tol=1e-9, max_cycles=60)
             assert info["cycles"] == oi["cycles"], (a, b)
             assert relmax(host(S.get_potential()), Po) <= 1e-12, (a, b)
+
+
+def test_full_size_per_iterate_parity(B, orc):
+    """BASELINE configs[2] at FULL size (257^3 fp64) in the launch configuration bench.py times (default flags:
+    temporally blocked finest level, fine-grained mid levels, shared-memory tail): the first V-cycle iterates are
+    compared element by element with the oracle (which needs ~0.3 s per cycle with OpenMP), C21."""
+    w = inputs.config(2)
+    with B.Solver.from_workload(w) as S:
+        S.solve_boundary(dev(w.Bz0, torch.float64))
+        P_or = host(S.get_potential())
+        c = 1.0 + w.f
+        for k in range(3):
+            info = S.solve_interior(tol=0.0, max_cycles=1)
+            P_or = orc.vcycle3(P_or, None, c, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
+            err = relmax(host(S.get_potential()), P_or)
+            assert err <= 1e-12, (k, err)
+        rk = orc.resnorm3(P_or, None, c, w.alpha, w.L)
+        assert abs(info["history"][0] - rk) <= 1e-6 * rk
 
 
 def test_large_grid_sampled_properties(B, orc):
