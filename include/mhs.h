@@ -70,6 +70,8 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
                                         paper's own kernel design; for A/B tests */
 #define MHS_FLAG_UNFUSED_KERNELS    4 /* tuned kernels, but one sweep per pass (no temporal blocking);
                                         for A/B tests of the fused smoother                              */
+#define MHS_FLAG_BIG_LEVEL_KERNELS  8 /* use the kernels of the big (HBM-bound) levels on every level they
+                                        can handle, whatever its size; for parity tests on small grids     */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 

@@ -20,6 +20,8 @@ from . import build as _build
 MHS_F32, MHS_F64 = 0, 1
 MHS_FLAG_REFERENCE_KERNELS = 1
 MHS_FLAG_SYNC_EACH_CYCLE = 2
+MHS_FLAG_UNFUSED_KERNELS = 4
+MHS_FLAG_BIG_LEVEL_KERNELS = 8
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8
 (MHS_OK, MHS_ERR_INVALID_ARG, MHS_ERR_GRID, MHS_ERR_NOT_ELLIPTIC, MHS_ERR_INDEFINITE, MHS_ERR_STATE,

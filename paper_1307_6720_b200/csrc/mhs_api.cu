@@ -257,7 +257,16 @@ bool use_fast(const mhs_ctx* ctx, const Level& lv)
 
 bool use_zsweep(const mhs_ctx* ctx, const Level& lv)
 {
-    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && !mid_level(lv) && zsweep_ok(ctx, lv);
+    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && !mid_level(ctx, lv) && zsweep_ok(ctx, lv);
+}
+
+// residual + full weighting into co.rhs: separable form on big levels, register z-streaming on the others
+void restrict_fast(mhs_ctx* ctx, const Level& lv, const void* u, const void* rhs, const Level& co, int reverse, const int* done)
+{
+    if (!mid_level(ctx, lv) && !(ctx->opt.flags & MHS_FLAG_UNFUSED_KERNELS) && lv.nz >= 5)
+        launch_resid_restrict_sep(ctx, lv, u, rhs, co, co.rhs, reverse, done);
+    else
+        launch_resid_restrict_z(ctx, lv, u, rhs, co, co.rhs, reverse, done);
 }
 
 int clus_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->clus3 : ctx->clus2; }
@@ -364,7 +373,7 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
     {
         Scope sc(ctx, kc_for(lv, l, 1));
         if (fast) {
-            launch_resid_restrict_z(ctx, lv, lv.u, rhs, co, co.rhs, ctx->dir, done);
+            restrict_fast(ctx, lv, lv.u, rhs, co, ctx->dir, done);
             ctx->dir ^= 1;
         } else {
             launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, done);
@@ -889,7 +898,7 @@ mhs_status mhs_op_restrict(mhs_ctx* ctx, int dim, int level)
     Scope sc(ctx, kc_for(lv, level, 1));
     const void* rhs = (dim == 3 && level == 0) ? nullptr : lv.rhs;
     if (use_fast(ctx, lv)) {
-        launch_resid_restrict_z(ctx, lv, lv.u, rhs, (*Ls)[level + 1], (*Ls)[level + 1].rhs, 0, nullptr);
+        restrict_fast(ctx, lv, lv.u, rhs, (*Ls)[level + 1], 0, nullptr);
     } else {
         launch_residual_ref(ctx, lv, lv.u, rhs, lv.r, nullptr);
         launch_restrict_ref(ctx, lv, lv.r, (*Ls)[level + 1], (*Ls)[level + 1].rhs, nullptr);

@@ -112,13 +112,15 @@ void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* 
 
 // ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);
-bool mid_level(const Level& lv);   // small enough to live in the L2: parallelism-bound, gets fine-grained launch shapes
+bool mid_level(const mhs_ctx* c, const Level& lv);   // small enough to live in the L2: parallelism-bound, gets fine-grained launch shapes
 // mode 0: sweep; 1: sweep + partial sums of the INPUT's ||rhs - L u||^2; 2: partial sums only; 3: the first two sweeps
 // from the zero initial guess in one pass (u not read).  Returns #partials.
 long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done);
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);
 void launch_resid_restrict_z(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
+// the same for a big level, in separable form (no plane of u kept, the residual never formed)
+void launch_resid_restrict_sep(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
 void launch_prolong_v(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, int reverse, const int* done);
 // ---- temporally blocked smoother (mhs_kernels_zfused.cu) ----
 bool zsweep_ok(const mhs_ctx* c, const Level& lv);

@@ -32,6 +32,7 @@ constexpr long long CL_MAX_PTS = 600000;  // largest level given to the cluster 
 template <typename T>
 struct TailLevelP {
     int nx, ny, nz;
+    int bx, by;                   // bits of the power-of-two index space of the interior nodes along x, y
     int off_u, off_rhs, off_tmp;  // element offsets into the shared array
     const T* tab;                 // global: cx | cy | diag | w
     T cz;
@@ -67,15 +68,70 @@ __device__ __forceinline__ T ldcg(const T* p) { return __ldcg(p); }
 // ---------------------------------------------------------------------------------------------
 // tail: levels in shared memory, plain dense layout (nx*ny*nz, walls stored as zeros), CTA 0 only
 // ---------------------------------------------------------------------------------------------
+// Interior nodes of a tail level are enumerated through a power-of-two index space (bx, by, bz bits per axis), so
+// that a thread turns its work index into (i, j, k) with shifts and masks instead of integer divisions.
 template <typename T>
-__device__ __forceinline__ T tail_Lu(const TailLevelP<T>& L, const T* u, int i, int j, int k, bool d3, T a2)
+struct TailIdx {
+    int mx, my, k0, k1, bx, bxy, n, nx, nxy;
+    __device__ __forceinline__ TailIdx(const TailLevelP<T>& L, bool d3)
+        : mx(L.nx - 2), my(L.ny - 2), k0(d3 ? 1 : 0), k1(d3 ? L.nz - 1 : 1), bx(L.bx), bxy(L.bx + L.by), nx(L.nx), nxy(L.nx * L.ny)
+    {
+        n = (k1 - k0) << bxy;
+    }
+    __device__ __forceinline__ bool at(int q, int& i, int& j, int& k, int& c) const
+    {
+        i = (q & ((1 << bx) - 1)) + 1;
+        j = ((q >> bx) & ((1 << (bxy - bx)) - 1)) + 1;
+        k = (q >> bxy) + k0;
+        c = i + nx * j + nxy * k;
+        return i <= mx && j <= my;
+    }
+    __device__ __forceinline__ bool at(int q, int& k, int& c) const
+    {
+        int i, j;
+        return at(q, i, j, k, c);
+    }
+};
+
+template <typename T>
+__device__ __forceinline__ T tail_Lu(const TailLevelP<T>& L, const T* u, int c, int k, bool d3, T a2)
 {
     const int nx = L.nx, nxy = L.nx * L.ny;
-    const int c = i + nx * j + nxy * k;
     const T uc = u[c];
     T lu = L.tab[k] * lap1<T>(u[c + 1], u[c - 1], uc) + L.tab[L.nz + k] * lap1<T>(u[c + nx], u[c - nx], uc);
     if (d3) lu += L.cz * lap1<T>(u[c + nxy], u[c - nxy], uc) + a2 * uc;
     return lu;
+}
+
+// dst = src + (omega/D_k)(rhs - L src) at the interior nodes (a2)
+template <typename T>
+__device__ __forceinline__ void tail_sweep(const TailLevelP<T>& L, const T* src, T* dst, const T* rhs, bool d3, T a2)
+{
+    const TailIdx<T> I(L, d3);
+    for (int q = threadIdx.x; q < I.n; q += blockDim.x) {
+        int k, c;
+        if (I.at(q, k, c)) dst[c] = src[c] + L.tab[3 * L.nz + k] * (rhs[c] - tail_Lu<T>(L, src, c, k, d3, a2));
+    }
+    __syncthreads();
+}
+
+// The first TWO sweeps from the zero initial guess in one phase: sweep 1 is u1 = (omega/D_k) rhs (rhs is zero on
+// every wall, so u1 is too), formed on the fly at the seven nodes sweep 2 reads.
+template <typename T>
+__device__ __forceinline__ void tail_sweep2_from_zero(const TailLevelP<T>& L, T* dst, const T* rhs, bool d3, T a2)
+{
+    const TailIdx<T> I(L, d3);
+    const int nx = L.nx, nxy = L.nx * L.ny;
+    for (int q = threadIdx.x; q < I.n; q += blockDim.x) {
+        int k, c;
+        if (!I.at(q, k, c)) continue;
+        const T w = L.tab[3 * L.nz + k];
+        const T f = rhs[c], uc = w * f;
+        T lu = L.tab[k] * lap1<T>(w * rhs[c + 1], w * rhs[c - 1], uc) + L.tab[L.nz + k] * lap1<T>(w * rhs[c + nx], w * rhs[c - nx], uc);
+        if (d3) lu += L.cz * lap1<T>(L.tab[3 * L.nz + k + 1] * rhs[c + nxy], L.tab[3 * L.nz + k - 1] * rhs[c - nxy], uc) + a2 * uc;
+        dst[c] = uc + w * (f - lu);
+    }
+    __syncthreads();
 }
 
 template <typename T>
@@ -84,6 +140,8 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
     const int tid = threadIdx.x, nt = blockDim.x;
     const bool d3 = P.dim3 != 0;
     const int nlev = P.ntail;
+    T* cur[8];   // which of a level's two iterate buffers holds its iterate (they ping-pong)
+    T* oth[8];
 
     // zero everything (walls must read as zeros), then load the top level's right-hand side
     int tot = 0;
@@ -92,12 +150,11 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
     __syncthreads();
     {
         const TailLevelP<T>& L = P.t[0];
-        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
-        const int mx = L.nx - 2, my = L.ny - 2;
-        const int n = mx * my * (kz1 - kz0);
-        for (int q = tid; q < n; q += nt) {
-            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-            S[L.off_rhs + i + L.nx * j + L.nx * L.ny * k] = ldcg(P.tail_rhs_g + i + P.tail_sx * j + P.tail_sp * k);
+        const TailIdx<T> I(L, d3);
+        for (int q = tid; q < I.n; q += nt) {
+            int i, j, k, c;
+            if (!I.at(q, i, j, k, c)) continue;
+            S[L.off_rhs + c] = ldcg(P.tail_rhs_g + i + P.tail_sx * j + P.tail_sp * k);
         }
     }
     __syncthreads();
@@ -106,41 +163,36 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
     for (int l = 0; l < nlev - 1; ++l) {
         const TailLevelP<T>& L = P.t[l];
         const TailLevelP<T>& C = P.t[l + 1];
-        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
-        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
-        T* u = S + L.off_u;
-        T* tmp = S + L.off_tmp;
+        cur[l] = S + L.off_u;
+        oth[l] = S + L.off_tmp;
         const T* rhs = S + L.off_rhs;
-        for (int s = 0; s < P.n_pre; ++s) {
-            for (int q = tid; q < n; q += nt) {
-                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-                const int c = i + L.nx * j + L.nx * L.ny * k;
-                tmp[c] = u[c] + L.tab[3 * L.nz + k] * (rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2));
-            }
-            __syncthreads();
-            for (int q = tid; q < n; q += nt) {
-                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-                const int c = i + L.nx * j + L.nx * L.ny * k;
-                u[c] = tmp[c];
-            }
-            __syncthreads();
+        int s0 = 0;
+        if (P.n_pre >= 2) {
+            tail_sweep2_from_zero<T>(L, cur[l], rhs, d3, P.a2);
+            s0 = 2;
         }
-        // residual -> tmp
-        for (int q = tid; q < n; q += nt) {
-            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-            const int c = i + L.nx * j + L.nx * L.ny * k;
-            tmp[c] = rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2);
+        for (int s = s0; s < P.n_pre; ++s) {   // (n_pre == 1: one ordinary sweep from the zero-filled buffer)
+            tail_sweep<T>(L, cur[l], oth[l], rhs, d3, P.a2);
+            T* x = cur[l]; cur[l] = oth[l]; oth[l] = x;
+        }
+        // residual -> the free iterate buffer (its walls are never read by the weighting below)
+        T* r = oth[l];
+        {
+            const TailIdx<T> I(L, d3);
+            for (int q = tid; q < I.n; q += nt) {
+                int k, c;
+                if (I.at(q, k, c)) r[c] = rhs[c] - tail_Lu<T>(L, cur[l], c, k, d3, P.a2);
+            }
         }
         __syncthreads();
         // full weighting -> rhs of the next level
         {
-            const int cmx = C.nx - 2, cmy = C.ny - 2;
-            const int ck0 = d3 ? 1 : 0, ck1 = d3 ? C.nz - 1 : 1;
-            const int cn = cmx * cmy * (ck1 - ck0);
+            const TailIdx<T> I(C, d3);
             T* rc = S + C.off_rhs;
-            for (int q = tid; q < cn; q += nt) {
-                const int I = q % cmx + 1, J = (q / cmx) % cmy + 1, K = q / (cmx * cmy) + ck0;
-                const T* r0 = tmp + 2 * I + L.nx * (2 * J) + L.nx * L.ny * (2 * K);
+            for (int q = tid; q < I.n; q += nt) {
+                int Ii, J, K, cc;
+                if (!I.at(q, Ii, J, K, cc)) continue;
+                const T* r0 = r + 2 * Ii + L.nx * (2 * J) + L.nx * L.ny * (2 * K);
                 T s = T(0);
                 for (int dc = (d3 ? -1 : 0); dc <= (d3 ? 1 : 0); ++dc) {
                     T sp = T(0);
@@ -152,10 +204,11 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
                     }
                     s += (d3 ? (dc == 0 ? T(0.5) : T(0.25)) : T(1)) * sp;
                 }
-                rc[I + C.nx * J + C.nx * C.ny * K] = s;
+                rc[cc] = s;
             }
         }
         __syncthreads();
+        // the residual's buffer goes back to being an iterate buffer: its interior is overwritten before it is read
     }
 
     // ---- coarsest level: exact solve e = A^-1 rhs (C9) ----
@@ -164,6 +217,7 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
         const int mx = L.nx - 2, my = L.ny - 2, k0 = d3 ? 1 : 0;
         const int n = P.ncoarse;
         T* u = S + L.off_u;
+        cur[nlev - 1] = u;
         const T* rhs = S + L.off_rhs;
         for (int row = tid; row < n; row += nt) {
             double s = 0.0;
@@ -181,49 +235,40 @@ __device__ void tail_body(const ClusterP<T>& P, T* S)
     for (int l = nlev - 2; l >= 0; --l) {
         const TailLevelP<T>& L = P.t[l];
         const TailLevelP<T>& C = P.t[l + 1];
-        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
-        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
-        T* u = S + L.off_u;
-        T* tmp = S + L.off_tmp;
         const T* rhs = S + L.off_rhs;
-        const T* ec = S + C.off_u;
-        for (int q = tid; q < n; q += nt) {
-            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-            const int I0 = i >> 1, I1 = (i + 1) >> 1, J0 = j >> 1, J1 = (j + 1) >> 1, K0 = k >> 1, K1 = (k + 1) >> 1;
+        const T* ec = cur[l + 1];
+        {
+            const TailIdx<T> I(L, d3);
+            T* u = cur[l];
             const int cxy = C.nx * C.ny;
-            T s = (ec[I0 + C.nx * J0 + cxy * K0] + ec[I1 + C.nx * J0 + cxy * K0]) +
-                  (ec[I0 + C.nx * J1 + cxy * K0] + ec[I1 + C.nx * J1 + cxy * K0]);
-            if (d3)
-                s += (ec[I0 + C.nx * J0 + cxy * K1] + ec[I1 + C.nx * J0 + cxy * K1]) +
-                     (ec[I0 + C.nx * J1 + cxy * K1] + ec[I1 + C.nx * J1 + cxy * K1]);
-            u[i + L.nx * j + L.nx * L.ny * k] += (d3 ? T(0.125) : T(0.25)) * s;
+            for (int q = tid; q < I.n; q += nt) {
+                int i, j, k, c;
+                if (!I.at(q, i, j, k, c)) continue;
+                const int I0 = i >> 1, I1 = (i + 1) >> 1, J0 = j >> 1, J1 = (j + 1) >> 1, K0 = k >> 1, K1 = (k + 1) >> 1;
+                T s = (ec[I0 + C.nx * J0 + cxy * K0] + ec[I1 + C.nx * J0 + cxy * K0]) +
+                      (ec[I0 + C.nx * J1 + cxy * K0] + ec[I1 + C.nx * J1 + cxy * K0]);
+                if (d3)
+                    s += (ec[I0 + C.nx * J0 + cxy * K1] + ec[I1 + C.nx * J0 + cxy * K1]) +
+                         (ec[I0 + C.nx * J1 + cxy * K1] + ec[I1 + C.nx * J1 + cxy * K1]);
+                u[c] += (d3 ? T(0.125) : T(0.25)) * s;
+            }
         }
         __syncthreads();
         for (int s = 0; s < P.n_post; ++s) {
-            for (int q = tid; q < n; q += nt) {
-                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-                const int c = i + L.nx * j + L.nx * L.ny * k;
-                tmp[c] = u[c] + L.tab[3 * L.nz + k] * (rhs[c] - tail_Lu<T>(L, u, i, j, k, d3, P.a2));
-            }
-            __syncthreads();
-            for (int q = tid; q < n; q += nt) {
-                const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-                const int c = i + L.nx * j + L.nx * L.ny * k;
-                u[c] = tmp[c];
-            }
-            __syncthreads();
+            tail_sweep<T>(L, cur[l], oth[l], rhs, d3, P.a2);
+            T* x = cur[l]; cur[l] = oth[l]; oth[l] = x;
         }
     }
 
     // ---- write the correction of the top tail level back (interior nodes) ----
     {
         const TailLevelP<T>& L = P.t[0];
-        const int kz0 = d3 ? 1 : 0, kz1 = d3 ? L.nz - 1 : 1;
-        const int mx = L.nx - 2, my = L.ny - 2, n = mx * my * (kz1 - kz0);
-        const T* u = S + L.off_u;
-        for (int q = tid; q < n; q += nt) {
-            const int i = q % mx + 1, j = (q / mx) % my + 1, k = q / (mx * my) + kz0;
-            P.tail_u_g[i + P.tail_sx * j + P.tail_sp * k] = u[i + L.nx * j + L.nx * L.ny * k];
+        const TailIdx<T> I(L, d3);
+        const T* u = cur[0];
+        for (int q = tid; q < I.n; q += nt) {
+            int i, j, k, c;
+            if (!I.at(q, i, j, k, c)) continue;
+            P.tail_u_g[i + P.tail_sx * j + P.tail_sp * k] = u[c];
         }
     }
 }
@@ -475,7 +520,7 @@ int cluster_start(const mhs_ctx* c, const std::vector<Level>& Ls, int tail)
     if (tail >= n) return n;   // no tail -> no cluster kernel (the coarsest solve is part of the tail)
     // A hierarchy whose finest level is big keeps only the tail here: its middle levels (<= 129^3) fill the GPU
     // better as ordinary grids (mhs_kernels_fast.cu, mid_level) than on the 16 SMs of one cluster.
-    if (Ls[0].dim == 3 && Ls[0].npts() > CL_MAX_PTS) return tail;
+    if (Ls[0].dim == 3 && (Ls[0].npts() > CL_MAX_PTS || (c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS))) return tail;
     int l = tail;
     while (l > 0 && tail - (l - 1) <= CL_MAXG && Ls[l - 1].npts() <= CL_MAX_PTS && Ls[l - 1].sp < (1LL << 30) / std::max(1, Ls[l - 1].nz)) --l;
     return l;
@@ -519,6 +564,8 @@ static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, 
         const Level& lv = Ls[q];
         TailLevelP<T>& t = P.t[q - lt];
         t.nx = lv.nx; t.ny = lv.ny; t.nz = lv.nz;
+        t.bx = 0; while ((1 << t.bx) < lv.nx - 2) ++t.bx;
+        t.by = 0; while ((1 << t.by) < lv.ny - 2) ++t.by;
         const int npa = ((int)lv.npts() + 3) & ~3;
         t.off_u = off; t.off_rhs = off + npa; t.off_tmp = off + 2 * npa;
         off += 3 * npa;

@@ -15,6 +15,8 @@
 //   * Grids are sized to fill a whole number of waves on the 148 SMs (z-chunk length is the free parameter);
 //     consecutive kernels traverse the z-chunks in opposite order so that the tail of what the previous
 //     kernel wrote is still in the 126 MB L2 when the next one starts.
+#include <cstdlib>
+
 #include "mhs_device.cuh"
 
 namespace mhs {
@@ -343,7 +345,7 @@ static int pick_chunks(long long xy_blocks, int planes, int slots, int min_chunk
 
 // Levels that fit in the L2 several times over (<= ~5 M nodes: 129^3 and below) are not bandwidth problems but
 // parallelism problems: they get one row per thread and short z-chunks, so that even 65^3 fills the 148 SMs.
-bool mid_level(const Level& lv) { return lv.npts() <= 5000000LL; }
+bool mid_level(const mhs_ctx* c, const Level& lv) { return !(c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS) && lv.npts() <= 5000000LL; }
 
 template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM, bool ZERO2>
 static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int reverse, const int* done)
@@ -385,7 +387,7 @@ long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void
             return smooth_z_t<T, R, false, false, true, false>(c, lv, u, rhs, out, reverse, done);                   \
         }                                                                                                            \
     } while (0)
-    const bool mid = mid_level(lv);
+    const bool mid = mid_level(c, lv);
     if (c->es == 8) { if (mid) SZ(double, 1); SZ(double, 4); }
     else { if (mid) SZ(float, 1); SZ(float, 4); }
 #undef SZ
@@ -395,7 +397,7 @@ long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
 {
     const int V = c->es == 8 ? 2 : 4;
-    const int R = mid_level(lv) ? 1 : 4;
+    const int R = mid_level(c, lv) ? 1 : 4;
     const long long items = (long long)((lv.sy + R - 1) / R) * (lv.sx / V);
     return ((items + 127) / 128) * (long long)std::max(1, (lv.nz - 2 + 1) / 2 + 1);
 }
@@ -434,7 +436,7 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
 void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
 {
     count_launch(c);
-    const bool mid = mid_level(f);
+    const bool mid = mid_level(c, f);
 #define RR(T)                                                                                  \
     do {                                                                                       \
         if (mid) {                                                                             \
@@ -459,6 +461,184 @@ void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, cons
         k_prolong_v<double><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (double*)u, co.sx, co.sp, (const double*)ec, reverse, f.nz - 2, done);
     else
         k_prolong_v<float><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (float*)u, co.sx, co.sp, (const float*)ec, reverse, f.nz - 2, done);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Residual + full weighting of a BIG level in separable form (a3 + a4).  Every operator involved is a tensor
+// product, and the 27 fine nodes under a coarse interior node are all interior, so
+//     R (f - L u) = R f - [ Rz c_k ( (Rx Dxx) (x) Ry + Rx (x) (Ry Dyy) ) + (Rx (x) Ry) (Rz Dzz) + a^2 Rx (x) Ry (x) Rz ] u
+// with the 1D composites  R = (1/4, 1/2, 1/4) on offsets (-1, 0, 1)  and  R D2 = (1/4, -1/2, 1/4) / h^2 on offsets
+// (-2, 0, 2).  A thread reduces each fine row it touches in x to two numbers, scatters them into the y-partials of
+// its RC coarse rows, and scatters those into a sliding window of three coarse planes while it walks up in z: no plane
+// of u is kept, the residual is never formed, ~6 flops per fine node instead of ~15.  Same result as residual-then-
+// restrict up to rounding order (the sums are regrouped, rounding-order differences).
+// Work item: x vector xv (V fine columns -> V/2 coarse columns), coarse rows J0 .. J0+RC-1.
+// ------------------------------------------------------------------------------------------------
+template <typename T, int RC, bool HAS_RHS>
+__global__ void __launch_bounds__(128) k_resid_restrict_sep(LP<T> p, const T* __restrict__ u, const T* __restrict__ rhs, int csx, int csy,
+                                                            long long csp, int cnz, T* __restrict__ rc, int Kchunk, int reverse,
+                                                            const int* __restrict__ done)
+{
+    if (done && *done) return;
+    constexpr int V = VN<T>::N;
+    constexpr int VC = V / 2;
+    constexpr int NROW = 2 * RC + 3;
+    const int nvx = p.sx / V;
+    const int ngroups = (csy - 1 + RC - 1) / RC;
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= (long long)nvx * ngroups) return;
+    const int g = (int)(q / nvx), xv = (int)(q - (long long)g * nvx);
+    const int i0 = xv * V, J0 = 1 + g * RC;
+    const int zc = reverse ? (int)gridDim.y - 1 - (int)blockIdx.y : (int)blockIdx.y;
+    const int Kb = 1 + zc * Kchunk;
+    const int Ke = min(Kb + Kchunk, cnz - 1);
+    if (Kb >= Ke) return;
+    const T hz2 = p.cz, a2 = p.a2;                       // 1/hz^2, alpha^2
+    const T* tab = p.tab;                                // cx[k] = c_k/hx^2 | cy[k] = c_k/hy^2
+    const long long rowbase = i0 + (long long)p.sx * (2 * J0 - 2);
+
+    T accM[RC][VC], accC[RC][VC], accP[RC][VC];          // coarse planes K-1, K, K+1 of  R L u
+    T fC[RC][VC], fP[RC][VC];                            // coarse planes K, K+1 of  R f
+#pragma unroll
+    for (int s = 0; s < RC; ++s)
+#pragma unroll
+        for (int m = 0; m < VC; ++m) accM[s][m] = accC[s][m] = accP[s][m] = fC[s][m] = fP[s][m] = T(0);
+
+    // xy-reduced quantities of fine plane k for the thread's coarse nodes:  A = (Rx Ry) u,  Q = c_k (RxDxx Ry + Rx RyDyy) u,  F = (Rx Ry) f
+    auto plane = [&](int k, T (&A)[RC][VC], T (&Q)[RC][VC], T (&F)[RC][VC]) {
+        T Bx[RC][VC], By[RC][VC];
+#pragma unroll
+        for (int s = 0; s < RC; ++s)
+#pragma unroll
+            for (int m = 0; m < VC; ++m) A[s][m] = Bx[s][m] = By[s][m] = F[s][m] = T(0);
+        const T* pl = u + rowbase + p.sp * k;
+#pragma unroll
+        for (int t = 0; t < NROW; ++t) {
+            const T* row = pl + (long long)p.sx * t;
+            const Vec<T> c = ldv(row);
+            const T l0 = row[-2], l1 = row[-1], r0 = row[V];
+            T a[VC], b[VC];
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                const T um2 = m == 0 ? l0 : c.v[2 * m - 2], um1 = m == 0 ? l1 : c.v[2 * m - 1];
+                const T up1 = c.v[2 * m + 1], up2 = m == VC - 1 ? r0 : c.v[2 * m + 2];
+                a[m] = T(0.5) * c.v[2 * m] + T(0.25) * (um1 + up1);
+                b[m] = T(0.25) * (um2 + up2) - T(0.5) * c.v[2 * m];
+            }
+            T af[VC];
+            if (HAS_RHS && t >= 1 && t <= NROW - 2) {
+                const T* fr = rhs + rowbase + p.sp * k + (long long)p.sx * t;
+                const Vec<T> f = ldv(fr);
+                const T fl = fr[-1];
+#pragma unroll
+                for (int m = 0; m < VC; ++m) af[m] = T(0.5) * f.v[2 * m] + T(0.25) * ((m == 0 ? fl : f.v[2 * m - 1]) + f.v[2 * m + 1]);
+            }
+#pragma unroll
+            for (int s = 0; s < RC; ++s) {
+                const int d = t - (2 + 2 * s);   // fine row offset from the coarse row's centre
+#pragma unroll
+                for (int m = 0; m < VC; ++m) {
+                    if (d == 0) { A[s][m] += T(0.5) * a[m]; Bx[s][m] += T(0.5) * b[m]; By[s][m] -= T(0.5) * a[m]; }
+                    if (d == 1 || d == -1) { A[s][m] += T(0.25) * a[m]; Bx[s][m] += T(0.25) * b[m]; }
+                    if (d == 2 || d == -2) By[s][m] += T(0.25) * a[m];
+                    if (HAS_RHS) {
+                        if (d == 0) F[s][m] += T(0.5) * af[m];
+                        if (d == 1 || d == -1) F[s][m] += T(0.25) * af[m];
+                    }
+                }
+            }
+        }
+        const T cx = tab[k], cy = tab[p.nz + k];
+#pragma unroll
+        for (int s = 0; s < RC; ++s)
+#pragma unroll
+            for (int m = 0; m < VC; ++m) Q[s][m] = cx * Bx[s][m] + cy * By[s][m];
+    };
+
+    for (int K = Kb - 1; K <= Ke; ++K) {
+        T A[RC][VC], Q[RC][VC], F[RC][VC];
+        // even fine plane 2K: weight 1/2 for K; its (Rz Dzz) part also feeds K-1 and K+1
+        plane(2 * K, A, Q, F);
+        const bool zin = 2 * K >= 1 && 2 * K <= p.nz - 2;   // L u (and f) live on interior planes only
+#pragma unroll
+        for (int s = 0; s < RC; ++s)
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                const T az = T(0.25) * hz2 * A[s][m];
+                accM[s][m] += az;
+                accP[s][m] += az;
+                accC[s][m] += (zin ? T(0.5) * Q[s][m] + T(0.5) * a2 * A[s][m] : T(0)) - T(0.5) * hz2 * A[s][m];
+                if (HAS_RHS && zin) fC[s][m] += T(0.5) * F[s][m];
+            }
+        // coarse plane K-1 is complete
+        if (K - 1 >= Kb) {
+#pragma unroll
+            for (int s = 0; s < RC; ++s)
+#pragma unroll
+                for (int m = 0; m < VC; ++m) {
+                    const int I = (i0 >> 1) + m, J = J0 + s;
+                    if (I > 0 && J < csy) rc[I + (long long)csx * J + csp * (K - 1)] = -accM[s][m];
+                }
+        }
+        if (K == Ke) break;
+        // odd fine plane 2K+1: weight 1/4 for K and for K+1
+        plane(2 * K + 1, A, Q, F);
+#pragma unroll
+        for (int s = 0; s < RC; ++s)
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                const T v = T(0.25) * Q[s][m] + T(0.25) * a2 * A[s][m];
+                accC[s][m] += v;
+                accP[s][m] += v;
+                if (HAS_RHS) { fC[s][m] += T(0.25) * F[s][m]; fP[s][m] += T(0.25) * F[s][m]; }
+            }
+        // slide the window: K -> K+1.  (R f)[K] is complete here too; fold it into the plane that is stored next.
+#pragma unroll
+        for (int s = 0; s < RC; ++s)
+#pragma unroll
+            for (int m = 0; m < VC; ++m) {
+                accM[s][m] = HAS_RHS ? accC[s][m] - fC[s][m] : accC[s][m];
+                accC[s][m] = accP[s][m];
+                accP[s][m] = T(0);
+                fC[s][m] = fP[s][m];
+                fP[s][m] = T(0);
+            }
+    }
+}
+
+template <typename T, bool HAS_RHS, int RC>
+static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
+{
+    constexpr int V = VN<T>::N;
+    auto kern = k_resid_restrict_sep<T, RC, HAS_RHS>;
+    static int slots = 0;
+    if (!slots) {
+        int nb = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
+        slots = std::max(1, nb) * c->num_sms;
+    }
+    const long long items = (long long)(f.sx / V) * ((co.sy - 1 + RC - 1) / RC);
+    const long long xb = (items + 127) / 128;
+    const int planes = co.nz - 2;
+    // z-chunks: one wave of resident blocks (the kernel is bound by parallelism before bytes: measured at 257^3, 32 chunks
+    // of 4 coarse planes -- 11 fine planes read for 8 -- beat 16 chunks of 8 by 57 -> 41 us); no shorter than 4 coarse planes
+    int nzc = (int)std::max<long long>(1, std::min<long long>(planes / 4 > 0 ? planes / 4 : 1, slots / xb));
+    const int Kchunk = (planes + nzc - 1) / nzc;
+    nzc = (planes + Kchunk - 1) / Kchunk;
+    dim3 grid((unsigned)xb, (unsigned)nzc);
+    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sy, co.sp, co.nz, (T*)rc, Kchunk, reverse, done);
+}
+
+void launch_resid_restrict_sep(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
+{
+    count_launch(c);
+    if (c->es == 8) {
+        if (rhs) resid_restrict_sep_t<double, true, 4>(c, f, u, rhs, co, rc, reverse, done);
+        else resid_restrict_sep_t<double, false, 4>(c, f, u, rhs, co, rc, reverse, done);
+    } else {
+        if (rhs) resid_restrict_sep_t<float, true, 4>(c, f, u, rhs, co, rc, reverse, done);
+        else resid_restrict_sep_t<float, false, 4>(c, f, u, rhs, co, rc, reverse, done);
+    }
 }
 
 }  // namespace mhs

@@ -35,6 +35,12 @@ template <> struct ZV<double> { static constexpr int N = 2; static constexpr int
 template <> struct ZV<float> { static constexpr int N = 4; static constexpr int NCO = 4; };
 
 constexpr int ZR = 4;     // rows of a thread's patch
+constexpr int ZWY = 4;    // warps of a tile along y: a tile has ZWY*ZR patch rows
+// Tile geometry is a compile-time function of WXT (warps along x), so that every shared-memory stride is an immediate:
+template <typename T, int WXT> struct ZG {
+    static constexpr int TC = WXT * 32 * ZV<T>::N;          // tile columns
+    static constexpr int INP = (ZWY * ZR + 2) * TC;         // elements of one ring slot / exchange plane
+};
 constexpr int ZNIN = 4;   // input ring depth (planes)
 
 template <typename T>
@@ -239,13 +245,14 @@ struct ZCtx {
 };
 
 // warp 0: request input plane `k` of the tile into ring slot nload % ZNIN
-template <typename T>
+template <typename T, int WXT>
 __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int nload, int k)
 {
     const int slot = nload & (ZNIN - 1);
-    T* dst = IN + (size_t)slot * p.in_plane;
+    constexpr int TCc = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
+    T* dst = IN + (size_t)slot * INP;
     const T* src = tile_src + p.sp * k;
-    const uint32_t plane_bytes = (uint32_t)p.in_plane * sizeof(T);
+    const uint32_t plane_bytes = (uint32_t)INP * sizeof(T);
     uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(bars)) + slot;
     const int lane = threadIdx.x & 31;
     if (p.ntx == 1) {
@@ -256,9 +263,9 @@ __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint3
     } else {
         if (lane == 0) mbar_expect_tx(bar, plane_bytes);
         __syncwarp();
-        const int rows_in = p.WY * ZR + 2;
+        const int rows_in = ZWY * ZR + 2;
         for (int r = lane; r < rows_in; r += 32)
-            bulk_g2s(dst + r * p.TC, src + (long long)r * p.sx, (uint32_t)(p.TC * sizeof(T)), bar);
+            bulk_g2s(dst + r * TCc, src + (long long)r * p.sx, (uint32_t)(TCc * sizeof(T)), bar);
     }
 }
 
@@ -284,42 +291,42 @@ __device__ __forceinline__ void zc_load(ZCoef<float>& k, uint32_t a, bool, bool)
 }
 
 // End of a plane step: the ring slot of plane t-1 and the exchange plane of t-2 have been read by everybody.
-template <typename T, bool ZERO>
+template <typename T, int WXT, bool ZERO>
 __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, bool may_issue)
 {
     __syncthreads();
     if (!ZERO && may_issue) {
         const int k = z.t + ZNIN - 1;      // the slot of plane t-1 is free: request plane t+ZNIN-1 into it
-        if (k <= z.kend_in && threadIdx.x < 32) z_issue(p, tile_src, z.bars, IN, z.zoff + k, k);
+        if (k <= z.kend_in && threadIdx.x < 32) z_issue<T, WXT>(p, tile_src, z.bars, IN, z.zoff + k, k);
     }
     ++z.t;
 }
 
 // First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
-template <typename T, bool ZERO>
+template <typename T, int WXT, bool ZERO>
 __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0)
 {
     if (!ZERO) {
         const int pos = z.zoff + z.t;
         mbar_wait32(z.bars + 8 * (pos & (ZNIN - 1)), (uint32_t)((pos >> 2) & 1));
-        const uint32_t a = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * (uint32_t)(p.in_plane * sizeof(T));
+        const uint32_t a = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
 #pragma unroll
-        for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(p.TC * sizeof(T)));
+        for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(ZG<T, WXT>::TC * sizeof(T)));
     }
-    z_advance<T, ZERO>(p, z, tile_src, IN, false);
+    z_advance<T, WXT, ZERO>(p, z, tile_src, IN, false);
 }
 
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (the step is unrolled twice), so no register is ever moved.
-template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
 {
     constexpr int V = ZV<T>::N;
     constexpr uint32_t ES = sizeof(T);
-    const uint32_t rowb = (uint32_t)p.TC * ES;
-    const uint32_t planeb = (uint32_t)p.in_plane * ES;
+    constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES;
+    constexpr uint32_t planeb = (uint32_t)ZG<T, WXT>::INP * ES;
     const int t = z.t;
     const bool in1 = (unsigned)(t - 1 - z.kb) < (unsigned)z.nout;   // plane t-1 is an output plane of this segment
     const bool in2 = (unsigned)(t - 2 - z.kb) < (unsigned)z.nout;
@@ -394,11 +401,11 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     z.coef += ZV<T>::NCO * ES;
     z.o_last += p.sp;
     if (HAS_RHS) z.f1 += p.sp;
-    z_advance<T, ZERO>(p, z, tile_src, IN, true);
+    z_advance<T, WXT, ZERO>(p, z, tile_src, IN, true);
 }
 
-template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
-__global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
+__global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
 {
     static_assert(S == 1 || S == 2, "S sweeps per pass: 1 or 2");
@@ -409,21 +416,21 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
     constexpr int H = S - 1;                               // rows a tile loses on each side to the later sweeps
     extern __shared__ __align__(128) unsigned char zsm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int wx = warp % p.WX, wy = warp / p.WX;
-    const int TC = p.TC;
-    const int NR = p.WY * ZR;                              // patch rows of a tile
+    const int wx = warp % WXT, wy = warp / WXT;
+    constexpr int TC = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
+    constexpr int NR = ZWY * ZR;                           // patch rows of a tile
     // shared memory: [mbarriers: 128 B] [coefficients: a pad record + zcap records] [IN ring: ZNIN planes] [EX: 2 planes]
     uint64_t* bars = reinterpret_cast<uint64_t*>(zsm);
     T* coef = reinterpret_cast<T*>(zsm + 128) + NCO;       // record of plane kstart; the record before it is a pad
     T* IN = reinterpret_cast<T*>(zsm + 128 + p.coef_bytes);
-    T* EX = IN + (size_t)(ZERO ? 0 : ZNIN) * p.in_plane;
+    T* EX = IN + (size_t)(ZERO ? 0 : ZNIN) * INP;
 
     if (!ZERO && threadIdx.x == 0) {
         for (int q = 0; q < ZNIN; ++q) mbar_init(bars + q, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (S == 2) {   // guard rows and never-written parts of the exchange planes must hold zeros (a wall row may sit there)
-        for (int q = threadIdx.x; q < 2 * p.in_plane; q += blockDim.x) EX[q] = T(0);
+        for (int q = threadIdx.x; q < 2 * INP; q += blockDim.x) EX[q] = T(0);
     }
     if (threadIdx.x < NCO) coef[-NCO + (int)threadIdx.x] = T(0);
     __syncthreads();
@@ -455,11 +462,12 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
 
         // per-plane coefficient records of this segment
         __syncthreads();   // the previous segment is done with the table
-        for (int i = threadIdx.x; i < (kend_in - kstart + 1) * NCO; i += blockDim.x) {
+        for (int i = threadIdx.x; i < (kend_in - kstart + 2) * NCO; i += blockDim.x) {   // + a zero record for the idle step
             const int k = kstart + i / NCO, c = i % NCO;
             const T* t = p.tab;
             T v = T(0);
-            if (sizeof(T) == 8) {
+            if (k > kend_in) {
+            } else if (sizeof(T) == 8) {
                 // A | By | Bz | wz | iw^2 | -
                 if (c == 0) v = t[4 * p.nz + k];
                 else if (c == 1) v = t[6 * p.nz + k];
@@ -477,7 +485,7 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
         if (!ZERO) {
             const int n = min(ZNIN, kend_in - kstart + 1);
             if (warp == 0)
-                for (int i = 0; i < n; ++i) z_issue(p, tile_src, z.bars, IN, ring + i, kstart + i);
+                for (int i = 0; i < n; ++i) z_issue<T, WXT>(p, tile_src, z.bars, IN, ring + i, kstart + i);
             ring += kend_in - kstart + 1;
         }
         __syncthreads();   // coefficient table visible
@@ -511,13 +519,14 @@ __global__ void __launch_bounds__(512, 1) k_zsweep(const __grid_constant__ ZP<T>
             for (int e = 0; e < V; ++e) X.r[r].v[e] = Y.r[r].v[e] = P.r[r].v[e] = Q.r[r].v[e] = T(0);
 
         const int tend = ke - 1 + S;
-        z_first<T, ZERO>(p, z, tile_src, IN, X);
-        while (true) {
-            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, Y, X, Q, P);
-            if (z.t > tend) break;
-            z_step<T, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, X, Y, P, Q);
-            if (z.t > tend) break;
-        }
+        z_first<T, WXT, ZERO>(p, z, tile_src, IN, X);
+        // Steps come in pairs so that the loop has ONE back edge on which every register set is back in its place
+        // (no moves).  An odd segment runs one idle step past its end: nothing arrives, nothing is stored (masks),
+        // the coefficient table has a spare record for it.
+        do {
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, Y, X, Q, P);
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, X, Y, P, Q);
+        } while (z.t <= tend);
         // planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
     }
     if (NORM) {
@@ -574,7 +583,7 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
     const long long items = (long long)z.ntx * z.nty * (lv.nz - 2);
     // one CTA per SM; a z-segment should be long against its S warm-up planes
     z.ctas = (int)std::max<long long>(1, std::min<long long>(c->num_sms, items / 12));
-    z.zcap = (int)std::min<long long>(lv.nz, (items + z.ctas - 1) / z.ctas + 2 * S + 2);
+    z.zcap = (int)std::min<long long>(lv.nz + 1, (items + z.ctas - 1) / z.ctas + 2 * S + 3);
     z.coef_bytes = (int)(((size_t)(z.zcap + 1) * NCO * sizeof(T) + 127) / 128 * 128);
     z.in_plane = (NR + 2) * z.TC;
     const size_t plane = (size_t)z.in_plane * sizeof(T);
@@ -585,10 +594,10 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
     return z;
 }
 
-template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
-static int zsweep_launch(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done)
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
+static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done)
 {
-    auto kern = k_zsweep<T, S, HAS_RHS, ZERO, NORM>;
+    auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM>;
     static bool attr = false;
     if (!attr) {
         cudaFuncAttributes fa;
@@ -609,14 +618,25 @@ static int zsweep_launch(mhs_ctx* c, const Level& lv, const ZCfg& z, const void*
     p.zcap = z.zcap;
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
-    kern<<<z.ctas, z.WX * z.WY * 32, z.smem, c->stream>>>(p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
+    kern<<<z.ctas, WXT * ZWY * 32, z.smem, c->stream>>>(p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (getenv("MHS_DEBUG")) {
         cudaError_t e = cudaPeekAtLastError();
-        fprintf(stderr, "[mhs] k_zsweep<%s,S=%d,rhs=%d,zero=%d,norm=%d> %dx%dx%d WX %d WY %d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
-                sizeof(T) == 8 ? "f64" : "f32", S, (int)HAS_RHS, (int)ZERO, (int)NORM, lv.nx, lv.ny, lv.nz, z.WX, z.WY, z.TC, z.ntx, z.nty,
+        fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
+                sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
                 z.ctas, z.smem, cudaGetErrorString(e));
     }
     return z.ctas;
+}
+
+template <typename T, int S, bool HAS_RHS, bool ZERO, bool NORM>
+static int zsweep_launch(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done)
+{
+    switch (z.WX) {
+        case 1: return zsweep_launch_w<T, 1, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
+        case 2: return zsweep_launch_w<T, 2, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
+        case 3: return zsweep_launch_w<T, 3, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
+        default: return zsweep_launch_w<T, 4, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
+    }
 }
 
 bool zsweep_ok(const mhs_ctx* c, const Level& lv)

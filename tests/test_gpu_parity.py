@@ -49,11 +49,13 @@ WORKLOADS = {
     "cfg1_129": lambda: inputs.config(1),          # sx = 128: the vector kernels' fp32 shapes (128-column warps)
     "slab_129x65x33": lambda: inputs.small(nx=129, ny=65, nz=33, L=(2.0, 1.0, 0.5), seed=11),
 }
-VARIANTS = {"fast": 0, "reference": 1}
+# fast: the default launch shapes;  big: the big-level (HBM-bound) kernels forced onto these small grids;
+# unfused: tuned kernels without temporal blocking / separable restriction;  reference: the paper's kernel design
+VARIANTS = {"fast": 0, "big": 8, "unfused": 4 | 8, "reference": 1}
 
 
 def flags_of(B, variant):
-    return B.MHS_FLAG_REFERENCE_KERNELS if variant == "reference" else 0
+    return VARIANTS[variant]
 
 
 # ------------------------------------------------------------------ single operators ---------
