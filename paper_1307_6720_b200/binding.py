@@ -262,9 +262,9 @@ class Solver:
         return cls(w.nx, w.ny, w.nz, w.L, w.alpha, w.f, dtype=kw.pop("dtype", dt), **kw)
 
     def close(self):
-        if getattr(self, "h", None):
-            mhs_destroy(self.h)
-            self.h = None
+        h, self.h = getattr(self, "h", None), None
+        if h and _lib is not None:      # (at interpreter exit the module may already be torn down)
+            _lib.mhs_destroy(h)
 
     __del__ = close
 

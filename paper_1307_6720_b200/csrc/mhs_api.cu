@@ -2,6 +2,7 @@
 // Host logic only -- every arithmetic step of the path runs in the kernels of mhs_kernels_*.cu.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 

@@ -309,7 +309,7 @@ template <typename T, bool D3>
 __device__ void ph_sweep(const GLevelP<T>& L, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ out, T a2, Who w)
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
-#pragma unroll 2
+#pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
         if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
@@ -323,7 +323,7 @@ template <typename T, bool D3>
 __device__ void ph_scale(const GLevelP<T>& L, const T* __restrict__ rhs, T* __restrict__ out, Who w)
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
-#pragma unroll 2
+#pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
         if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
@@ -346,7 +346,7 @@ template <typename T, bool D3>
 __device__ void ph_residual(const GLevelP<T>& L, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ r, T a2, Who w)
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
-#pragma unroll 2
+#pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
         if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
@@ -361,7 +361,7 @@ __device__ double ph_resnorm(const GLevelP<T>& L, const T* __restrict__ u, const
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
     double acc = 0.0;
-#pragma unroll 2
+#pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
         if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
@@ -402,7 +402,7 @@ template <typename T, bool D3>
 __device__ void ph_prolong(const GLevelP<T>& L, T* __restrict__ u, const T* __restrict__ ec, int csx, int csp, Who w)
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
-#pragma unroll 2
+#pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
         if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
@@ -591,7 +591,9 @@ static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, 
     if (P.nglob > 0) {
         // enough CTAs that a phase of the largest cluster level is a handful of row segments per warp
         const long long items = Ls[lc].npts() / 32;
-        ncta = items > 4096 ? c->cluster_max : items > 1024 ? std::min(8, c->cluster_max) : items > 256 ? 4 : 2;
+        // (measured: the 257^2 solve takes 3.5 / 2.2 / 1.55 / 1.2 ms on 2 / 4 / 8 / 16 CTAs -- phases are chains of L2 round trips,
+        // so every halving of the items per thread pays)
+        ncta = items > 512 ? c->cluster_max : items > 128 ? std::min(8, c->cluster_max) : items > 32 ? 4 : 2;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)ncta);
