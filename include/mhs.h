@@ -125,7 +125,10 @@ void mhs_default_options(mhs_options *o);
 /* Build a context: level hierarchy (C8), per-level coefficient tables c_l[k] = 1 + f(z_k) injected
  * to the coarse levels (C7), omega/D_k, inverse of the coarsest operators (C9), device arrays.
  * f_profile: host, nz doubles, f(z_k) at the nodes (NULL -> 0: the force-free case).
- * bc: NULL or all MHS_BC_DIRICHLET_ZERO.  opts: NULL -> defaults.  P is initialised to 0 (step 1). */
+ * bc: NULL or all MHS_BC_DIRICHLET_ZERO.  opts: NULL -> defaults.  P is initialised to 0 (step 1).
+ * grid->nz == 1 makes a BOUNDARY-ONLY context: only eq (11) on the nx x ny plane is set up (step 2 of the
+ * procedure); mhs_solve_boundary works and its result is read with mhs_level_get(ctx, 2, 0, 0, P0),
+ * the interior / field calls return MHS_ERR_STATE. */
 mhs_status mhs_create(const mhs_grid *grid, double alpha, const double *f_profile, const mhs_bc *bc,
                       const mhs_options *opts, mhs_ctx **out);
 void mhs_destroy(mhs_ctx *ctx);

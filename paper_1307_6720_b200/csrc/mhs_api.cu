@@ -576,9 +576,10 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         !(o.mu0 > 0.0) || o.g == 0.0 || o.boundary_max_cycles < 1 || !(grid->Lx > 0 && grid->Ly > 0 && grid->Lz > 0))
         return fail(ctx, MHS_ERR_INVALID_ARG, "invalid option value");
     const int ext[3] = {grid->nx, grid->ny, grid->nz};
-    for (int a = 0; a < 3; ++a)
+    const bool only2d = grid->nz == 1;   // boundary-only context: eq (11) on the plane, no interior (mhs.h, mhs_create)
+    for (int a = 0; a < (only2d ? 2 : 3); ++a)
         if (ext[a] < 3 || ((ext[a] - 1) & 1))
-            return fail(ctx, MHS_ERR_GRID, "every extent must be 2^m*q+1 with m >= 1 (an even number >= 2 of intervals)");
+            return fail(ctx, MHS_ERR_GRID, "every extent must be 2^m*q+1 with m >= 1 (an even number >= 2 of intervals); nz = 1 = 2D only");
     const int nz = grid->nz;
     ctx->f.assign(nz, 0.0);
     if (f_profile) ctx->f.assign(f_profile, f_profile + nz);
@@ -589,7 +590,7 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     if (o.rho_b) ctx->rho_b.assign(o.rho_b, o.rho_b + nz);
     const double hz = grid->Lz / (nz - 1);
     if (o.dfdz) ctx->dfdz.assign(o.dfdz, o.dfdz + nz);
-    else {  // C14: central differences of the samples, one-sided second order at both ends
+    else if (!only2d) {  // C14: central differences of the samples, one-sided second order at both ends
         const std::vector<double>& f = ctx->f;
         for (int k = 1; k < nz - 1; ++k) ctx->dfdz[k] = (f[k + 1] - f[k - 1]) / (2.0 * hz);
         ctx->dfdz[0] = (-3.0 * f[0] + 4.0 * f[1] - f[2]) / (2.0 * hz);
@@ -603,9 +604,9 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         return fail(ctx, MHS_ERR_CUDA, "no CUDA device: libmhs_b200 has no CPU fallback");
     }
     mhs_status st;
-    if ((st = build_hierarchy(ctx, 3, ctx->L3))) return st;
+    if (!only2d && (st = build_hierarchy(ctx, 3, ctx->L3))) return st;
     if ((st = build_hierarchy(ctx, 2, ctx->L2))) return st;
-    if (ctx->L3.size() < 2) return fail(ctx, MHS_ERR_GRID, "the 3D hierarchy needs at least two levels (>= 4 intervals per axis, max_levels != 1)");
+    if (!only2d && ctx->L3.size() < 2) return fail(ctx, MHS_ERR_GRID, "the 3D hierarchy needs at least two levels (>= 4 intervals per axis, max_levels != 1)");
 
     std::vector<double> ft(4 * (size_t)nz);
     for (int k = 0; k < nz; ++k) {
@@ -623,12 +624,13 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ctx->num_sms = pr.multiProcessorCount;
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
-    ctx->tail3 = ref ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
+    ctx->tail3 = (ref || only2d) ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
     ctx->tail2 = ref ? (int)ctx->L2.size() : tail_start(ctx, ctx->L2, 216 * 1024);
-    ctx->clus3 = ref ? (int)ctx->L3.size() : cluster_start(ctx, ctx->L3, ctx->tail3);
+    ctx->clus3 = (ref || only2d) ? (int)ctx->L3.size() : cluster_start(ctx, ctx->L3, ctx->tail3);
     ctx->clus2 = ref ? (int)ctx->L2.size() : cluster_start(ctx, ctx->L2, ctx->tail2);
     if (!ref) ctx->cluster_max = cluster_max_size(ctx);
-    ctx->npartial = std::max<long long>(64, std::max(resnorm_partial_capacity(ctx->L3[0]), resnorm_partial_capacity(ctx->L2[0])));
+    ctx->npartial = std::max<long long>(64, resnorm_partial_capacity(ctx->L2[0]));
+    if (!only2d) ctx->npartial = std::max(ctx->npartial, resnorm_partial_capacity(ctx->L3[0]));
     for (const Level& lv : ctx->L3) ctx->npartial = std::max(ctx->npartial, smooth_z_partial_capacity(ctx, lv));
     ctx->npartial = std::max<long long>(ctx->npartial, 4 * ctx->num_sms);
     CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
@@ -664,14 +666,17 @@ mhs_status mhs_solve_boundary(mhs_ctx* ctx, const void* Bz0, mhs_solve_info* inf
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (!Bz0) return fail(ctx, MHS_ERR_INVALID_ARG, "Bz0 is NULL");
-    if (ctx->L3.empty() || ctx->L2.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
-    Level& l3 = ctx->L3[0];
+    if (ctx->L2.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    const bool have3 = !ctx->L3.empty();
+    Level& l3 = have3 ? ctx->L3[0] : ctx->L2[0];   // (a 2D-only context has no interior to fill)
     Level& l2 = ctx->L2[0];
     {
         Scope sc(ctx, MHS_KC_PACK);
         // step 1: P = 0 everywhere
-        CK(cudaMemsetAsync(field_base(ctx, l3, l3.u), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
-        CK(cudaMemsetAsync(field_base(ctx, l3, l3.tmp), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
+        if (have3) {
+            CK(cudaMemsetAsync(field_base(ctx, l3, l3.u), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
+            CK(cudaMemsetAsync(field_base(ctx, l3, l3.tmp), 0, (size_t)l3.alloc * ctx->es, ctx->stream));
+        }
         CK(cudaMemsetAsync(field_base(ctx, l2, l2.u), 0, (size_t)l2.alloc * ctx->es, ctx->stream));
         if (l2.tmp) CK(cudaMemsetAsync(field_base(ctx, l2, l2.tmp), 0, (size_t)l2.alloc * ctx->es, ctx->stream));
         launch_pack(ctx, l2, Bz0, l2.rhs, true, true);  // rhs2 = -Bz0 at interior nodes (eq 11)
@@ -681,13 +686,13 @@ mhs_status mhs_solve_boundary(mhs_ctx* ctx, const void* Bz0, mhs_solve_info* inf
     // step 2
     mhs_status st = run_cycles(ctx, ctx->L2, ctx->opt.boundary_tol, ctx->opt.boundary_max_cycles, 0.0, info);
     if (st != MHS_OK && st != MHS_ERR_NOT_CONVERGED) return st;
-    {
+    if (have3) {
         Scope sc(ctx, MHS_KC_PACK);
         // P(:,:,0) = P0, in both ping-pong buffers of the finest 3D level (same in-plane layout)
         CK(cudaMemcpyAsync(l3.u, ctx->L2[0].u, (size_t)l2.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
         CK(cudaMemcpyAsync(l3.tmp, ctx->L2[0].u, (size_t)l2.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
     }
-    ctx->have_boundary = true;
+    ctx->have_boundary = have3;
     return st;
 }
 
@@ -720,6 +725,7 @@ mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solv
 mhs_status mhs_get_potential(mhs_ctx* ctx, void* P)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
     if (!P) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
     Scope sc(ctx, MHS_KC_PACK);
     launch_unpack(ctx, ctx->L3[0], ctx->L3[0].u, P);
@@ -730,6 +736,7 @@ mhs_status mhs_get_potential(mhs_ctx* ctx, void* P)
 mhs_status mhs_get_potential_host(mhs_ctx* ctx, void* P_host)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
     if (!P_host) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
     const size_t bytes = (size_t)ctx->L3[0].npts() * ctx->es;
     mhs_status st = ensure_stage(ctx, bytes);
@@ -743,6 +750,7 @@ mhs_status mhs_get_potential_host(mhs_ctx* ctx, void* P_host)
 mhs_status mhs_set_potential(mhs_ctx* ctx, const void* P)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
     if (!P) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
     Level& l3 = ctx->L3[0];
     Scope sc(ctx, MHS_KC_PACK);
@@ -774,6 +782,7 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
 mhs_status mhs_fields_host(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
     const size_t nb = (size_t)ctx->L3[0].npts() * ctx->es;
     mhs_status st = ensure_stage(ctx, 5 * nb);
     if (st) return st;

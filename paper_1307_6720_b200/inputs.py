@@ -166,10 +166,10 @@ def config(index: int, shrink: int = 1, replica: int = 0) -> Workload:
 
 def boundary_only(n: int = 4097, L: float = 4.0, patches: int = 256, dtype: str = "f32") -> Workload:
     """The 2D-only timing case of configs[4]: eq (11) on an n x n plane (domain [0,L]^2, same
-    patch recipe, seed index 5).  nz = 3 is a dummy interior that is never solved."""
+    patch recipe, seed index 5).  nz = 1: a boundary-only context (include/mhs.h, mhs_create)."""
     rng = SplitMix64(SEED_BASE + 5)
     bz = random_patches(rng, patches, n, n, L, L, 0.01, 0.05)
-    w = Workload(name="boundary%d" % n, nx=n, ny=n, nz=3, Lx=L, Ly=L, Lz=1.0, alpha=0.0, a=0.0,
+    w = Workload(name="boundary%d" % n, nx=n, ny=n, nz=1, Lx=L, Ly=L, Lz=1.0, alpha=0.0, a=0.0,
                  kappa=0.0, dtype=dtype, tol=1e-6 if dtype == "f32" else 1e-10)
     w.Bz0 = bz - bz.mean()
     return _finish(w)

@@ -48,6 +48,7 @@ WORKLOADS = {
     "cfg3_v33_65": lambda: inputs.config(3, shrink=8),
     "cfg1_129": lambda: inputs.config(1),          # sx = 128: the vector kernels' fp32 shapes (128-column warps)
     "slab_129x65x33": lambda: inputs.small(nx=129, ny=65, nz=33, L=(2.0, 1.0, 0.5), seed=11),
+    "cfg4_129x129x33": lambda: inputs.config(4, shrink=8),   # coarsest level 9x9x3: a 49-unknown exact solve
 }
 # fast: the default launch shapes;  big: the big-level (HBM-bound) kernels forced onto these small grids;
 # unfused: tuned kernels without temporal blocking / separable restriction;  reference: the paper's kernel design
@@ -332,6 +333,26 @@ def test_odd_sweep_counts_and_v11(B, orc):
             Po, oi = orc.solve_interior(P, w.f, w.alpha, w.L, omega=w.omega, n_pre=a, n_post=b, tol=1e-9, max_cycles=60)
             assert info["cycles"] == oi["cycles"], (a, b)
             assert relmax(host(S.get_potential()), Po) <= 1e-12, (a, b)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_boundary_only_context(B, orc, dtype):
+    """nz = 1: the 2D problem alone (BASELINE configs[4], "time the 2D boundary Poisson MG alone"), here at 1025^2 so
+    that the oracle's 16 cycles take well under a second.  Levels above 513^2 run as ordinary grids, the rest in the
+    cluster kernel; fp32 stops on the stagnation rule (C20) and is held to 1e-5 of the converged fp64 oracle."""
+    w = inputs.boundary_only(1025, dtype="f32" if dtype == torch.float32 else "f64")
+    with B.Solver.from_workload(w, dtype=dtype) as S:
+        info = S.solve_boundary(dev(w.Bz0, dtype))
+        P0 = host(S.level_get(2, 0, 0))
+        Po, ob = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly), omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=1e-10)
+        assert info["converged"]
+        if dtype == torch.float64:
+            assert info["cycles"] == ob["cycles"]
+        assert relmax(P0, Po) <= TOL[dtype]
+        for call in (lambda: S.solve_interior(1e-10, 5), lambda: S.fields(), lambda: S.get_potential()):
+            with pytest.raises(B.MHSError) as e:
+                call()
+            assert e.value.status == B.MHS_ERR_STATE
 
 
 def test_full_size_per_iterate_parity(B, orc):
