@@ -6,7 +6,11 @@
 //     of memory, so the input planes are brought in by the bulk-copy engine (cp.async.bulk global -> shared,
 //     completion on an mbarrier: the TMA data path without a tensor map) into a ring of NIN planes, several
 //     planes ahead of the arithmetic; no register or thread is spent on prefetching.
-//   * A CTA owns a tile of WY*4 rows x TC columns and walks up in z.  Stage s of the pipeline lags one plane
+//   * "Few fat threads": a thread owns 8 rows x one vector (ZR = 8, 256 threads per CTA, up to 255 registers), and the
+//     shared-memory operands of a row are fetched one row ahead of its arithmetic.  Measured at 257^3: 4 rows x 512 threads
+//     x 128 registers 68 us per 2-sweep pass, the same with row-ahead loads 66 us (ptxas sinks the loads back to their uses
+//     when registers are short), 8 rows x 256 threads x 254 registers 62.5 us -- latency is hidden by ILP, not by warps.
+//   * A CTA owns a tile of ZWY*ZR rows x TC columns and walks up in z.  Stage s of the pipeline lags one plane
 //     behind stage s-1: at step t stage 1 makes sweep-1 values of plane t-1 from the input planes t-2, t-1, t,
 //     stage 2 makes sweep-2 values of plane t-2 from sweep-1 planes t-3, t-2, t-1.  A thread owns a patch of
 //     4 rows x one 128-bit vector and keeps the z-column (below, centre, above) of its patch for every stage in
@@ -34,8 +38,8 @@ template <typename T> struct ZV;
 template <> struct ZV<double> { static constexpr int N = 2; static constexpr int NCO = 6; };
 template <> struct ZV<float> { static constexpr int N = 4; static constexpr int NCO = 4; };
 
-constexpr int ZR = 4;     // rows of a thread's patch
-constexpr int ZWY = 4;    // warps of a tile along y: a tile has ZWY*ZR patch rows
+constexpr int ZR = 8;     // rows of a thread's patch
+constexpr int ZWY = 2;    // warps of a tile along y: a tile has ZWY*ZR patch rows
 // Tile geometry is a compile-time function of WXT (warps along x), so that every shared-memory stride is an immediate:
 template <typename T, int WXT> struct ZG {
     static constexpr int TC = WXT * 32 * ZV<T>::N;          // tile columns
@@ -344,24 +348,49 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     const int m1 = in1 ? z.omask : 0, m2 = in2 ? z.omask : 0;
     double pa = 0.0;
     float pf = 0.f;
+    // Everything a row needs from memory, fetched ONE ROW AHEAD of the arithmetic (the loop is fully unrolled, so the
+    // two sets are just names): the loads of row r+1 are in flight while row r is computed, instead of each row
+    // exposing a shared-memory round trip at its first use.
+    struct RowIn {
+        ZVec<T> up0, edge1, edge2, f1, f2;
+        T w, e, w2, e2;
+    };
+    auto load_row = [&](int r, RowIn& q) {
+        const long long grow = (long long)r * p.sx;
+        if (!ZERO) {
+            q.up0 = lds_vec<T>(a_new + r * rowb);
+            q.w = lds_one<T>(a_cen + r * rowb - ES);
+            q.e = lds_one<T>(a_cen + r * rowb + V * ES);
+            if (r == ZR - 1) q.edge1 = lds_vec<T>(a_cen + ZR * rowb);
+            if (r == 0) q.edge1 = lds_vec<T>(a_cen - rowb);
+        }
+        if (HAS_RHS) q.f1 = zld(z.f1 + grow);
+        if (S == 2) {
+            q.w2 = lds_one<T>(a_exr + r * rowb - ES);
+            q.e2 = lds_one<T>(a_exr + r * rowb + V * ES);
+            if (r == ZR - 1) q.edge2 = lds_vec<T>(a_exr + ZR * rowb);
+            if (r == 0) q.edge2 = lds_vec<T>(a_exr - rowb);
+            if (HAS_RHS) q.f2 = zld(z.f1 - p.sp + grow);
+        }
+    };
+    RowIn rin[2];
+    load_row(0, rin[0]);
 #pragma unroll
     for (int r = 0; r < ZR; ++r) {
         const long long grow = (long long)r * p.sx;
+        RowIn& in = rin[r & 1];
+        if (r + 1 < ZR) load_row(r + 1, rin[(r + 1) & 1]);
         // ---------------- stage 1: sweep-1 values of row r of plane t-1 ----------------
-        ZVec<T> up0, o1, f1;
-        if (!ZERO) up0 = lds_vec<T>(a_new + r * rowb);
-        if (HAS_RHS) f1 = zld(z.f1 + grow);
+        ZVec<T> o1;
         if (ZERO) {
 #pragma unroll
-            for (int e = 0; e < V; ++e) o1.v[e] = k1.wz * f1.v[e];
+            for (int e = 0; e < V; ++e) o1.v[e] = k1.wz * in.f1.v[e];
             if (z.cw0) o1.v[0] = T(0);
         } else {
-            const T w = lds_one<T>(a_cen + r * rowb - ES), e = lds_one<T>(a_cen + r * rowb + V * ES);
-            ZVec<T> nn, ss;
-            if (r == ZR - 1) nn = lds_vec<T>(a_cen + ZR * rowb); else nn = c0.r[r + 1 < ZR ? r + 1 : r];
-            if (r == 0) ss = lds_vec<T>(a_cen - rowb); else ss = c0.r[r > 0 ? r - 1 : 0];
+            const ZVec<T> nn = r == ZR - 1 ? in.edge1 : c0.r[r + 1 < ZR ? r + 1 : r];
+            const ZVec<T> ss = r == 0 ? in.edge1 : c0.r[r > 0 ? r - 1 : 0];
             float rs = 0.f;
-            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], w, e, nn, ss, up0, dn0.r[r], f1, o1, z.cw0, rs);
+            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], in.w, in.e, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
             if (z.cw0) o1.v[0] = c0.r[r].v[0];
             if (NORM && (m1 & (1 << r))) {
                 if (sizeof(T) == 8) {
@@ -374,21 +403,18 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
                     pf += rs;
                 }
             }
-            dn0.r[r] = up0;     // becomes the centre plane of the next step
+            dn0.r[r] = in.up0;     // becomes the centre plane of the next step
         }
         if (S == 1) {
             if (m1 & (1 << r)) zst(z.o_last + grow, o1);
         } else {
             sts_vec(a_exw + r * rowb, o1);
             // ---------------- stage 2: sweep-2 values of row r of plane t-2 ----------------
-            ZVec<T> o2, f2;
-            if (HAS_RHS) f2 = zld(z.f1 - p.sp + grow);
-            const T w = lds_one<T>(a_exr + r * rowb - ES), e = lds_one<T>(a_exr + r * rowb + V * ES);
-            ZVec<T> nn, ss;
-            if (r == ZR - 1) nn = lds_vec<T>(a_exr + ZR * rowb); else nn = c1.r[r + 1 < ZR ? r + 1 : r];
-            if (r == 0) ss = lds_vec<T>(a_exr - rowb); else ss = c1.r[r > 0 ? r - 1 : 0];
+            ZVec<T> o2;
+            const ZVec<T> nn = r == ZR - 1 ? in.edge2 : c1.r[r + 1 < ZR ? r + 1 : r];
+            const ZVec<T> ss = r == 0 ? in.edge2 : c1.r[r > 0 ? r - 1 : 0];
             float rs;
-            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], w, e, nn, ss, o1, dn1.r[r], f2, o2, false, rs);
+            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], in.w2, in.e2, nn, ss, o1, dn1.r[r], in.f2, o2, false, rs);
             if (z.cw0) o2.v[0] = c1.r[r].v[0];
             if (m2 & (1 << r)) zst(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
@@ -547,7 +573,7 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
 // ------------------------------------------------------------------------------------------------
 struct ZCfg {
     bool ok = false;
-    int WX = 0, WY = 4, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
+    int WX = 0, WY = ZWY, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
     size_t smem = 0;
 };
 
@@ -561,7 +587,7 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
     const int lane_cols = 32 * V;
     if (lv.sx % lane_cols != 0) return z;
     const int wfull = lv.sx / lane_cols;
-    z.WY = 4;
+    z.WY = ZWY;
     const int NR = z.WY * ZR;
     if (lv.sy < NR + 1) return z;
     if (wfull <= 4) {
