@@ -246,25 +246,40 @@ def main():
     S.reset_profile()
     ms_e2e, _, _, c3_all_e2e, _ = timed(True, args.steps)
 
-    # ---- roofline of the dominant kernel: the finest-level smoother ----
+    # ---- roofline of the dominant kernel: k_zsweep, the temporally blocked finest-level smoother.
+    # It runs as two kinds of launch: plain passes (class smooth_l0: read u, write u', S sweeps) and prolongation-fused
+    # post-smoothing passes (class prolong_l0 when fused_prolong_l0 > 0: read u and e_c, write u').  Algorithmic bytes
+    # per launch: 2w per node, + w/8 for the coarse correction; whatever the number of sweeps fused in it.
     peak, peak_src = peaks()
     n_int = (w.nx - 2) * (w.ny - 2) * (w.nz - 2)
-    launches = prof["launches"]["smooth_l0"]
     sweeps = prof["sweeps_l0"]
-    t_smooth_ms = prof["ms"]["smooth_l0"]
-    # algorithmic bytes: read u + write u' once per launch, whatever the number of sweeps fused in it
-    # (2w/s per update, s sweeps per launch) -> 2*w*n_int per launch
-    bytes_per_launch = 2.0 * es * n_int
-    achieved = bytes_per_launch * launches / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0
-    traffic = read_traffic("smooth_l0_dram_bytes_per_launch_%d" % w.nx)
-    roof = {"bound": "hbm", "kernel": "finest-level weighted-Jacobi smoother (kernel class smooth_l0)",
+    l_plain, t_plain = prof["launches"]["smooth_l0"], prof["ms"]["smooth_l0"]
+    l_fused = prof["fused_prolong_l0"]
+    fused_all = l_fused > 0 and l_fused == prof["launches"]["prolong_l0"]
+    t_fused = prof["ms"]["prolong_l0"] if fused_all else 0.0
+    b_plain, b_fused = 2.0 * es * n_int, (2.0 + 0.125) * es * n_int
+    launches = l_plain + (l_fused if fused_all else 0)
+    t_smooth_ms = t_plain + t_fused
+    alg_bytes = b_plain * l_plain + (b_fused * l_fused if fused_all else 0.0)
+    achieved = alg_bytes / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0
+    tr_p = read_traffic("smooth_l0_dram_bytes_per_launch_%d" % w.nx)
+    tr_f = read_traffic("prolong_smooth_l0_dram_bytes_per_launch_%d" % w.nx)
+    traffic = tr_p
+    if fused_all and tr_p is not None and tr_f is not None and launches:
+        traffic = (tr_p * l_plain + tr_f * l_fused) / launches
+    roof = {"bound": "hbm", "kernel": "k_zsweep: finest-level weighted-Jacobi smoother, 2 sweeps per HBM pass "
+                                      "(plain passes + prolongation-fused post-smoothing passes)",
             "achieved": achieved, "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak,
             "frac_of_8TBs_nominal": achieved / 8000.0, "traffic": traffic,
             "launches": launches, "sweeps": sweeps, "sweeps_per_launch": (sweeps / launches) if launches else None,
             "avg_launch_us": 1e3 * t_smooth_ms / launches if launches else None,
-            "algorithmic_bytes_per_launch": bytes_per_launch,
+            "algorithmic_bytes_per_launch": alg_bytes / launches if launches else None,
             "smoother_gpts_per_s": n_int * sweeps / (t_smooth_ms * 1e-3) / 1e9 if t_smooth_ms > 0 else 0.0,
-            "smoother_share_of_step": t_smooth_ms / ms}
+            "smoother_share_of_step": t_smooth_ms / ms,
+            "plain_pass": {"launches": l_plain, "avg_us": 1e3 * t_plain / l_plain if l_plain else None,
+                           "algorithmic_bytes": b_plain, "gbs": b_plain * l_plain / (t_plain * 1e-3) / 1e9 if t_plain > 0 else None},
+            "prolong_fused_pass": ({"launches": l_fused, "avg_us": 1e3 * t_fused / l_fused, "algorithmic_bytes": b_fused,
+                                    "gbs": b_fused * l_fused / (t_fused * 1e-3) / 1e9} if fused_all and t_fused > 0 else None)}
 
     out = {"metric": METRIC, "value": c3_all / (ms * 1e-3), "unit": "V-cycles/s", "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",

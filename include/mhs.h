@@ -72,6 +72,8 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
                                         for A/B tests of the fused smoother                              */
 #define MHS_FLAG_BIG_LEVEL_KERNELS  8 /* use the kernels of the big (HBM-bound) levels on every level they
                                         can handle, whatever its size; for parity tests on small grids     */
+#define MHS_FLAG_SEPARATE_PROLONG  16 /* keep the prolongation a pass of its own instead of folding it into the
+                                        first post-smoothing pass of the big levels; for A/B tests              */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 
@@ -104,7 +106,8 @@ typedef struct {
 enum {
     MHS_KC_SMOOTH_L0 = 0,   /* Jacobi sweeps on the finest 3D level (the dominant, HBM-bound kernel) */
     MHS_KC_RESTRICT_L0 = 1, /* residual + full weighting on the finest 3D level                      */
-    MHS_KC_PROLONG_L0 = 2,  /* trilinear correction on the finest 3D level                           */
+    MHS_KC_PROLONG_L0 = 2,  /* trilinear correction on the finest 3D level (alone, or fused with the
+                               first post-smoothing pass: see mhs_profile.fused_prolong_l0)          */
     MHS_KC_NORM_L0 = 3,     /* residual norm on the finest 3D level                                  */
     MHS_KC_COARSE_3D = 4,   /* everything on 3D levels >= 1                                          */
     MHS_KC_BOUNDARY_2D = 5, /* the whole 2D solve                                                    */
@@ -114,8 +117,11 @@ enum {
 };
 typedef struct {
     long long launches[MHS_KC_COUNT]; /* kernels launched per class since create / reset             */
-    double ms[MHS_KC_COUNT];          /* CUDA-event time per class (only with options.profile = 1)   */
+    double ms[MHS_KC_COUNT];          /* CUDA-event time per class (options.profile = 1: the smoothing and
+                                         prolongation classes of the finest level only; 2: every class)  */
     long long sweeps_l0;              /* Jacobi sweeps applied to the finest 3D level                */
+    long long fused_prolong_l0;       /* launches of class MHS_KC_PROLONG_L0 that were prolongation-fused
+                                         smoothing passes (prolongation + the first post-sweeps in one pass) */
 } mhs_profile;
 
 /* Fill *o with the defaults: fp64, omega 2/3, V(2,2), full coarsening, boundary_tol 1e-10,

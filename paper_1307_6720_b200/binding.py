@@ -22,6 +22,7 @@ MHS_FLAG_REFERENCE_KERNELS = 1
 MHS_FLAG_SYNC_EACH_CYCLE = 2
 MHS_FLAG_UNFUSED_KERNELS = 4
 MHS_FLAG_BIG_LEVEL_KERNELS = 8
+MHS_FLAG_SEPARATE_PROLONG = 16
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8
 (MHS_OK, MHS_ERR_INVALID_ARG, MHS_ERR_GRID, MHS_ERR_NOT_ELLIPTIC, MHS_ERR_INDEFINITE, MHS_ERR_STATE,
@@ -60,7 +61,7 @@ class mhs_solve_info(C.Structure):
 
 class mhs_profile(C.Structure):
     _fields_ = [("launches", C.c_longlong * MHS_KC_COUNT), ("ms", C.c_double * MHS_KC_COUNT),
-                ("sweeps_l0", C.c_longlong)]
+                ("sweeps_l0", C.c_longlong), ("fused_prolong_l0", C.c_longlong)]
 
 
 class MHSError(RuntimeError):
@@ -235,6 +236,7 @@ def mhs_get_profile(h):
     names = [lib().mhs_kernel_class_name(k).decode() for k in range(MHS_KC_COUNT)]
     return dict(launches={n: int(p.launches[k]) for k, n in enumerate(names)},
                 ms={n: float(p.ms[k]) for k, n in enumerate(names)}, sweeps_l0=int(p.sweeps_l0),
+                fused_prolong_l0=int(p.fused_prolong_l0),
                 total_launches=int(sum(p.launches)))
 
 

@@ -36,7 +36,7 @@ struct Scope {
     Scope(mhs_ctx* ctx, int kc) : c(ctx), prev(ctx->cur_kc)
     {
         c->cur_kc = kc;
-        timed = c->opt.profile >= 2 || (c->opt.profile == 1 && kc == MHS_KC_SMOOTH_L0);
+        timed = c->opt.profile >= 2 || (c->opt.profile == 1 && (kc == MHS_KC_SMOOTH_L0 || kc == MHS_KC_PROLONG_L0));
         if (timed) {
             ev.kc = kc;
             ev.a = take();
@@ -382,7 +382,20 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
         }
     }
     vcycle(ctx, Ls, l + 1, done);
-    {
+    int n_post = ctx->opt.n_post;
+    bool fused_prolong = false;
+    if (zs && n_post >= 1 && !(ctx->opt.flags & MHS_FLAG_SEPARATE_PROLONG)) {
+        // prolongation + correction folded into the first post-smoothing pass (no pass of its own over u)
+        Scope sc(ctx, kc_for(lv, l, 2));
+        const int S = std::min(2, n_post);
+        fused_prolong = launch_zsweep_prolong(ctx, lv, lv.u, rhs, lv.tmp, S, co, co.u, done);
+        if (fused_prolong) {
+            std::swap(lv.u, lv.tmp);
+            if (lv.dim == 3 && l == 0) { ctx->prof.sweeps_l0 += S; ctx->prof.fused_prolong_l0 += 1; }
+            n_post -= S;
+        }
+    }
+    if (!fused_prolong) {
         Scope sc(ctx, kc_for(lv, l, 2));
         if (fast) {
             launch_prolong_v(ctx, lv, lv.u, co, co.u, ctx->dir, done);
@@ -391,7 +404,7 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
             launch_prolong_ref(ctx, lv, lv.u, co, co.u, done);
         }
     }
-    smooth(ctx, Ls, l, ctx->opt.n_post, done);
+    smooth(ctx, Ls, l, n_post, done);
 }
 
 // Report a finished solve loop from the control block read back into ctx->ctl_host.

@@ -128,6 +128,11 @@ bool zsweep_ok(const mhs_ctx* c, const Level& lv);
 // squared residual of u go to c->partial; returns their number.
 int launch_zsweep(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, bool zero, bool norm, const int* done);
 
+// the same applied to u + P e_c (prolongation + correction folded into the pass; u is not modified).  false: not launched
+// (the level's tiles are not full rows) -- the caller prolongs separately.
+bool launch_zsweep_prolong(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, const Level& coarse, const void* ec,
+                           const int* done);
+
 // ---- the small-level cluster kernel (mhs_kernels_cluster.cu) ----
 int tail_start(const mhs_ctx* c, const std::vector<Level>& Ls, size_t budget_bytes);
 int cluster_start(const mhs_ctx* c, const std::vector<Level>& Ls, int tail);

@@ -44,8 +44,16 @@ constexpr int ZWY = 2;    // warps of a tile along y: a tile has ZWY*ZR patch ro
 template <typename T, int WXT> struct ZG {
     static constexpr int TC = WXT * 32 * ZV<T>::N;          // tile columns
     static constexpr int INP = (ZWY * ZR + 2) * TC;         // elements of one ring slot / exchange plane
+    // prolongation-fused variant (full-row tiles only): the coarse rows under the ZWY*ZR+2 fine rows of a tile
+    static constexpr int CSX = TC / 2;                      // coarse row pitch
+    static constexpr int CROWS = ZWY * ZR / 2 + 2;
+    static constexpr int CINP = CROWS * CSX + 16 / (int)sizeof(T);   // + the element after the last row (16-byte granule)
 };
-constexpr int ZNIN = 4;   // input ring depth (planes)
+constexpr int ZNIN = 4;   // input ring depth (planes); 3 in the prolongation-fused variant (shared memory pays for the coarse ring)
+constexpr int ZNCE = 3;   // coarse-correction ring depth (planes), prolongation-fused variant only
+
+template <int NIN> __device__ __forceinline__ int ring_slot(int pos) { return NIN == 4 ? (pos & 3) : pos % NIN; }
+template <int NIN> __device__ __forceinline__ uint32_t ring_par(int pos) { return NIN == 4 ? (uint32_t)((pos >> 2) & 1) : (uint32_t)((pos / NIN) & 1); }
 
 template <typename T>
 struct __align__(16) ZVec {
@@ -69,6 +77,8 @@ struct ZP {
     int NP;             // interior planes nz-2
     long long items;    // ntx*nty*NP
     int zcap;           // planes of the shared coefficient table
+    const T* ec;        // prolongation-fused variant: the coarse-grid correction (aliased layout, pitch sx/2), else null
+    long long csp;      //   its plane stride
     int in_plane;       // elements of one ring slot: (WY*ZR + 2) rows x TC (also the size of an exchange plane)
     int coef_bytes;     // bytes reserved for the coefficient table (multiple of 128)
 };
@@ -246,13 +256,18 @@ struct ZCtx {
     int omask;                    // rows of the patch that are stored (output rows, output columns)
     bool cw0;                     // element 0 of the patch is a wall column
     double acc;
+    // prolongation-fused variant
+    uint32_t in_base, ce_base;    // shared-space addresses of ring slot 0 / coarse ring slot 0
+    uint32_t ce_own;              // byte offset, inside a coarse slot, of (coarse row jrow0>>1, coarse column of element 0)
+    int czoff, cnext;             // ring position of coarse plane K is czoff + K; next coarse plane to request
+    int jt, Jb;                   // first patch row of the tile; first coarse row held in a coarse slot
 };
 
-// warp 0: request input plane `k` of the tile into ring slot nload % ZNIN
-template <typename T, int WXT>
+// warp 0: request input plane `k` of the tile into ring slot nload % NIN
+template <typename T, int WXT, int NIN>
 __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int nload, int k)
 {
-    const int slot = nload & (ZNIN - 1);
+    const int slot = ring_slot<NIN>(nload);
     constexpr int TCc = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
     T* dst = IN + (size_t)slot * INP;
     const T* src = tile_src + p.sp * k;
@@ -270,6 +285,30 @@ __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint3
         const int rows_in = ZWY * ZR + 2;
         for (int r = lane; r < rows_in; r += 32)
             bulk_g2s(dst + r * TCc, src + (long long)r * p.sx, (uint32_t)(TCc * sizeof(T)), bar);
+    }
+}
+
+// Prolongation-fused variant, warp 0: make sure every coarse plane up to the one fine plane `kfine` needs has been requested.
+// Coarse plane K (rows Jb .. Jb+CROWS-1, contiguous: full-row tiles) goes to coarse slot (czoff + K) % ZNCE; its mbarrier
+// follows the NIN barriers of the input ring.
+template <typename T, int WXT, int NIN>
+__device__ __forceinline__ void c_request(const ZP<T>& p, ZCtx<T>& z, int kfine)
+{
+    constexpr int CINP = ZG<T, WXT>::CINP, CSX = ZG<T, WXT>::CSX;
+    const int klast = min(kfine, p.nz - 2);
+    if (klast < 1) return;
+    const int kneed = (klast + 1) >> 1;
+    while (z.cnext <= kneed) {
+        if (threadIdx.x == 0) {
+            const int cpos = z.czoff + z.cnext;
+            const int slot = cpos % ZNCE;
+            uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + NIN + slot;
+            T* dst = reinterpret_cast<T*>(__cvta_shared_to_generic(z.ce_base)) + (size_t)slot * CINP;
+            const T* src = p.ec + p.csp * z.cnext + (long long)CSX * z.Jb;
+            mbar_expect_tx(bar, (uint32_t)(CINP * sizeof(T)));
+            bulk_g2s(dst, src, (uint32_t)(CINP * sizeof(T)), bar);
+        }
+        ++z.cnext;
     }
 }
 
@@ -295,35 +334,118 @@ __device__ __forceinline__ void zc_load(ZCoef<float>& k, uint32_t a, bool, bool)
 }
 
 // End of a plane step: the ring slot of plane t-1 and the exchange plane of t-2 have been read by everybody.
-template <typename T, int WXT, bool ZERO>
+template <typename T, int WXT, bool ZERO, bool PRO>
 __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, bool may_issue)
 {
+    constexpr int NIN = PRO ? 3 : ZNIN;
     __syncthreads();
     if (!ZERO && may_issue) {
-        const int k = z.t + ZNIN - 1;      // the slot of plane t-1 is free: request plane t+ZNIN-1 into it
-        if (k <= z.kend_in && threadIdx.x < 32) z_issue<T, WXT>(p, tile_src, z.bars, IN, z.zoff + k, k);
+        const int k = z.t + NIN - 1;      // the slot of plane t-1 is free: request plane t+NIN-1 into it
+        if (k <= z.kend_in) {
+            if (threadIdx.x < 32) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, z.zoff + k, k);
+            if (PRO) c_request<T, WXT, NIN>(p, z, k);
+        }
     }
     ++z.t;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Prolongation-fused variant, "stage 0": the trilinear correction u += P e_c (a6) is applied to input plane t IN PLACE in
+// its ring slot as soon as it has arrived -- own patch rows by their owner, the two halo rows of the tile by one vector
+// per thread -- so that the sweeps read corrected values everywhere and the separate prolongation pass (read u, write u)
+// disappears.  Nobody but the owner reads plane t's slot before the barrier that ends the step.  Interior planes, rows and
+// columns only (walls and the planes k = 0, nz-1 carry no correction).  Coarse operands come from the coarse ring.
+//   u(i,j,k) += 1/8 * sum over the 2x2x2 coarse nodes ((i,i+1)>>1, (j,j+1)>>1, (k,k+1)>>1)
+// ------------------------------------------------------------------------------------------------
+template <typename T, int WXT, int JP>
+__device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, uint32_t c0a, uint32_t c1a)
+{
+    constexpr int V = ZV<T>::N, VC = V / 2;
+    constexpr uint32_t ES = sizeof(T);
+    constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES, crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
+    constexpr int NJ = (JP + ZR) / 2 + 1;          // coarse rows under the ZR patch rows
+    T cz[NJ][VC + 1];                              // the two coarse planes summed
+#pragma unroll
+    for (int q = 0; q < NJ; ++q)
+#pragma unroll
+        for (int m = 0; m <= VC; ++m)
+            cz[q][m] = lds_one<T>(c0a + z.ce_own + q * crowb + m * ES) + lds_one<T>(c1a + z.ce_own + q * crowb + m * ES);
+#pragma unroll
+    for (int r = 0; r < ZR; ++r) {
+        const int q0 = (JP + r) >> 1, q1 = (JP + r + 1) >> 1;
+        ZVec<T> a = lds_vec<T>(a_pl + r * rowb);
+        T c[VC + 1];
+#pragma unroll
+        for (int m = 0; m <= VC; ++m) c[m] = cz[q0][m] + cz[q1][m];
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+            const T sum = (e & 1) ? (c[e >> 1] + c[(e >> 1) + 1]) : T(2) * c[e >> 1];
+            if (e > 0 || !z.cw0) a.v[e] += T(0.125) * sum;
+        }
+        sts_vec(a_pl + r * rowb, a);
+    }
+}
+
+template <typename T, int WXT, int NIN>
+__device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int t, int slot)
+{
+    constexpr int V = ZV<T>::N, VC = V / 2;
+    constexpr uint32_t ES = sizeof(T);
+    constexpr int TC = ZG<T, WXT>::TC, NR = ZWY * ZR;
+    constexpr uint32_t planeb = (uint32_t)ZG<T, WXT>::INP * ES, cplaneb = (uint32_t)ZG<T, WXT>::CINP * ES;
+    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
+    if (t < 1 || t > p.nz - 2) return;
+    const int K0 = t >> 1, K1 = (t + 1) >> 1;
+    const int p0 = z.czoff + K0, p1 = z.czoff + K1;
+    mbar_wait32(z.bars + 8 * (NIN + p0 % ZNCE), (uint32_t)((p0 / ZNCE) & 1));
+    mbar_wait32(z.bars + 8 * (NIN + p1 % ZNCE), (uint32_t)((p1 / ZNCE) & 1));
+    const uint32_t c0a = z.ce_base + (uint32_t)(p0 % ZNCE) * cplaneb, c1a = z.ce_base + (uint32_t)(p1 % ZNCE) * cplaneb;
+    const uint32_t a_pl = z.in_own + (uint32_t)slot * planeb;
+    if (z.jt & 1) z_prolong_rows<T, WXT, 1>(z, a_pl, c0a, c1a);     // (patch rows start ZR-aligned from jt: same parity)
+    else z_prolong_rows<T, WXT, 0>(z, a_pl, c0a, c1a);
+    // the halo rows of the tile (fine rows jt-1 and jt+NR): one vector per thread
+    const int nvr = TC / V;
+    const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
+    const int jh = which ? z.jt + NR : z.jt - 1;
+    if (jh >= 1 && jh < p.sy) {
+        const uint32_t a = z.in_base + (uint32_t)slot * planeb + (uint32_t)(((which ? NR + 1 : 0) * TC + hv * V) * ES);
+        const uint32_t co = (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)ES);
+        const uint32_t dj = (jh & 1) ? crowb : 0u;      // J1 = J0 + (j odd)
+        ZVec<T> v = lds_vec<T>(a);
+        T c[VC + 1];
+#pragma unroll
+        for (int m = 0; m <= VC; ++m)
+            c[m] = (lds_one<T>(c0a + co + m * ES) + lds_one<T>(c1a + co + m * ES)) +
+                   (lds_one<T>(c0a + co + dj + m * ES) + lds_one<T>(c1a + co + dj + m * ES));
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+            const T sum = (e & 1) ? (c[e >> 1] + c[(e >> 1) + 1]) : T(2) * c[e >> 1];
+            if (e > 0 || hv > 0) v.v[e] += T(0.125) * sum;
+        }
+        sts_vec(a, v);
+    }
+}
+
 // First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
-template <typename T, int WXT, bool ZERO>
+template <typename T, int WXT, bool ZERO, bool PRO>
 __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0)
 {
+    constexpr int NIN = PRO ? 3 : ZNIN;
     if (!ZERO) {
         const int pos = z.zoff + z.t;
-        mbar_wait32(z.bars + 8 * (pos & (ZNIN - 1)), (uint32_t)((pos >> 2) & 1));
-        const uint32_t a = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
+        mbar_wait32(z.bars + 8 * ring_slot<NIN>(pos), ring_par<NIN>(pos));
+        if (PRO) z_prolong<T, WXT, NIN>(p, z, z.t, ring_slot<NIN>(pos));
+        const uint32_t a = z.in_own + (uint32_t)ring_slot<NIN>(pos) * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
 #pragma unroll
         for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(ZG<T, WXT>::TC * sizeof(T)));
     }
-    z_advance<T, WXT, ZERO>(p, z, tile_src, IN, false);
+    z_advance<T, WXT, ZERO, PRO>(p, z, tile_src, IN, false);
 }
 
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (the step is unrolled twice), so no register is ever moved.
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
 {
@@ -337,11 +459,13 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     const bool fresh = !ZERO && t <= z.kend_in;                      // a new input plane arrives in this step
     const int pos = z.zoff + t;
     // !fresh (only the step after the top plane): the slot holds an older plane -- finite numbers that meet Bz = 0
-    const uint32_t a_new = z.in_own + (uint32_t)(pos & (ZNIN - 1)) * planeb;          // plane t
-    const uint32_t a_cen = z.in_own + (uint32_t)((pos - 1) & (ZNIN - 1)) * planeb;    // plane t-1
+    constexpr int NIN = PRO ? 3 : ZNIN;
+    const uint32_t a_new = z.in_own + (uint32_t)ring_slot<NIN>(pos) * planeb;          // plane t
+    const uint32_t a_cen = z.in_own + (uint32_t)ring_slot<NIN>(pos - 1) * planeb;      // plane t-1
     const uint32_t a_exw = z.ex_own + (uint32_t)(t & 1) * planeb;                      // sweep-1 plane t-1 (written now)
     const uint32_t a_exr = z.ex_own + (uint32_t)((t & 1) ^ 1) * planeb;                // sweep-1 plane t-2 (written a step ago)
-    if (fresh) mbar_wait32(z.bars + 8 * (pos & (ZNIN - 1)), (uint32_t)((pos >> 2) & 1));
+    if (fresh) mbar_wait32(z.bars + 8 * ring_slot<NIN>(pos), ring_par<NIN>(pos));
+    if (PRO && fresh) z_prolong<T, WXT, NIN>(p, z, t, ring_slot<NIN>(pos));
     ZCoef<T> k1, k2;
     zc_load(k1, z.coef, HAS_RHS, NORM);
     if (S == 2) zc_load(k2, z.coef - ZV<T>::NCO * ES, HAS_RHS, false);
@@ -427,15 +551,17 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     z.coef += ZV<T>::NCO * ES;
     z.o_last += p.sp;
     if (HAS_RHS) z.f1 += p.sp;
-    z_advance<T, WXT, ZERO>(p, z, tile_src, IN, true);
+    z_advance<T, WXT, ZERO, PRO>(p, z, tile_src, IN, true);
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
 __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
 {
     static_assert(S == 1 || S == 2, "S sweeps per pass: 1 or 2");
     static_assert(!ZERO || HAS_RHS, "a zero iterate with a zero right-hand side stays zero");
+    static_assert(!PRO || (!ZERO && !NORM), "the prolongation-fused pass is a post-smoothing pass");
+    constexpr int NIN = PRO ? 3 : ZNIN;
     if (done && *done) return;
     constexpr int V = ZV<T>::N;
     constexpr int NCO = ZV<T>::NCO;
@@ -445,14 +571,16 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
     const int wx = warp % WXT, wy = warp / WXT;
     constexpr int TC = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
     constexpr int NR = ZWY * ZR;                           // patch rows of a tile
-    // shared memory: [mbarriers: 128 B] [coefficients: a pad record + zcap records] [IN ring: ZNIN planes] [EX: 2 planes]
+    // shared memory: [mbarriers: 128 B] [coefficients: a pad record + zcap records] [IN ring: NIN planes] [EX: 2 planes]
+    // [PRO: coarse ring, ZNCE planes]
     uint64_t* bars = reinterpret_cast<uint64_t*>(zsm);
     T* coef = reinterpret_cast<T*>(zsm + 128) + NCO;       // record of plane kstart; the record before it is a pad
     T* IN = reinterpret_cast<T*>(zsm + 128 + p.coef_bytes);
-    T* EX = IN + (size_t)(ZERO ? 0 : ZNIN) * INP;
+    T* EX = IN + (size_t)(ZERO ? 0 : NIN) * INP;
+    T* CE = EX + (size_t)2 * INP;
 
     if (!ZERO && threadIdx.x == 0) {
-        for (int q = 0; q < ZNIN; ++q) mbar_init(bars + q, 1);
+        for (int q = 0; q < NIN + (PRO ? ZNCE : 0); ++q) mbar_init(bars + q, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (S == 2) {   // guard rows and never-written parts of the exchange planes must hold zeros (a wall row may sit there)
@@ -467,7 +595,11 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
     z.in_own = smem_u32(IN + (wy * ZR + 1) * TC + cx0);
     z.ex_own = smem_u32(EX + (wy * ZR + 1) * TC + cx0);
     z.acc = 0.0;
+    z.in_base = smem_u32(IN);
+    z.ce_base = PRO ? smem_u32(CE) : 0u;
+    z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0;
     int ring = 0;                                           // planes requested so far by this CTA (ring position)
+    int cring = 0;                                          // coarse planes requested so far (PRO)
     const long long q0 = p.items * blockIdx.x / gridDim.x, q1 = p.items * (blockIdx.x + 1) / gridDim.x;
 
     for (long long q = q0; q < q1;) {
@@ -509,10 +641,20 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
         }
         z.zoff = ring - kstart;
         if (!ZERO) {
-            const int n = min(ZNIN, kend_in - kstart + 1);
+            const int n = min(NIN, kend_in - kstart + 1);
             if (warp == 0)
-                for (int i = 0; i < n; ++i) z_issue<T, WXT>(p, tile_src, z.bars, IN, ring + i, kstart + i);
+                for (int i = 0; i < n; ++i) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, ring + i, kstart + i);
             ring += kend_in - kstart + 1;
+            if (PRO) {
+                // coarse planes (kfirst >> 1) .. ((klast + 1) >> 1) serve the corrected fine planes kfirst .. klast
+                z.jt = jt;
+                z.Jb = (jt - 1) >> 1;
+                const int kfirst = max(kstart, 1), klast = min(kend_in, p.nz - 2);
+                z.cnext = kfirst >> 1;
+                z.czoff = cring - z.cnext;
+                if (klast >= kfirst) cring += ((klast + 1) >> 1) - z.cnext + 1;
+                c_request<T, WXT, NIN>(p, z, kstart + n - 1);
+            }
         }
         __syncthreads();   // coefficient table visible
 
@@ -533,6 +675,7 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
         z.kb = kb;
         z.nout = ke - kb;
         z.kend_in = kend_in;
+        if (PRO) z.ce_own = (uint32_t)((((jrow0 >> 1) - z.Jb) * ZG<T, WXT>::CSX + (icol0 >> 1)) * (int)sizeof(T));
         z.coef = smem_u32(coef);
         // the first z_step runs at t = kstart+1: sweep 1 makes plane kstart, sweep 2 plane kstart-1
         z.f1 = rhs + own + p.sp * kstart;
@@ -545,13 +688,13 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
             for (int e = 0; e < V; ++e) X.r[r].v[e] = Y.r[r].v[e] = P.r[r].v[e] = Q.r[r].v[e] = T(0);
 
         const int tend = ke - 1 + S;
-        z_first<T, WXT, ZERO>(p, z, tile_src, IN, X);
+        z_first<T, WXT, ZERO, PRO>(p, z, tile_src, IN, X);
         // Steps come in pairs so that the loop has ONE back edge on which every register set is back in its place
         // (no moves).  An odd segment runs one idle step past its end: nothing arrives, nothing is stored (masks),
         // the coefficient table has a spare record for it.
         do {
-            z_step<T, WXT, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, Y, X, Q, P);
-            z_step<T, WXT, S, HAS_RHS, ZERO, NORM>(p, z, tile_src, IN, X, Y, P, Q);
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>(p, z, tile_src, IN, Y, X, Q, P);
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>(p, z, tile_src, IN, X, Y, P, Q);
         } while (z.t <= tend);
         // planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
     }
@@ -578,7 +721,7 @@ struct ZCfg {
 };
 
 template <typename T>
-static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
+static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro = false)
 {
     constexpr int V = ZV<T>::N;
     constexpr int NCO = ZV<T>::NCO;
@@ -614,16 +757,21 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero)
     z.in_plane = (NR + 2) * z.TC;
     const size_t plane = (size_t)z.in_plane * sizeof(T);
     const size_t limit = 227 * 1024 - 256;   // the kernel also has a little static shared memory
-    z.smem = 128 + z.coef_bytes + (zero ? 0 : ZNIN * plane) + 2 * plane;
+    z.smem = 128 + z.coef_bytes + (zero ? 0 : (pro ? 3 : ZNIN) * plane) + 2 * plane;
+    if (pro) {   // full-row tiles only: the coarse rows under a tile are then one contiguous chunk per plane
+        if (z.ntx != 1 || zero) return z;
+        z.smem += (size_t)ZNCE * (((NR / 2 + 2) * (z.TC / 2) + 16 / sizeof(T)) * sizeof(T));
+    }
     if (z.smem > limit) return z;
     z.ok = true;
     return z;
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM>
-static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done)
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO = false>
+static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done,
+                           const void* ec = nullptr, long long csp = 0)
 {
-    auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM>;
+    auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>;
     static bool attr = false;
     if (!attr) {
         cudaFuncAttributes fa;
@@ -644,11 +792,12 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.zcap = z.zcap;
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
+    p.ec = (const T*)ec; p.csp = csp;
     kern<<<z.ctas, WXT * ZWY * 32, z.smem, c->stream>>>(p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (getenv("MHS_DEBUG")) {
         cudaError_t e = cudaPeekAtLastError();
-        fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
-                sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
+        fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
+                sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, (int)PRO, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
                 z.ctas, z.smem, cudaGetErrorString(e));
     }
     return z.ctas;
@@ -663,6 +812,40 @@ static int zsweep_launch(mhs_ctx* c, const Level& lv, const ZCfg& z, const void*
         case 3: return zsweep_launch_w<T, 3, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
         default: return zsweep_launch_w<T, 4, S, HAS_RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done);
     }
+}
+
+template <typename T, int S, bool HAS_RHS>
+static void zsweep_launch_pro(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done,
+                              const void* ec, long long csp)
+{
+    switch (z.WX) {
+        case 1: zsweep_launch_w<T, 1, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        case 2: zsweep_launch_w<T, 2, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        case 3: zsweep_launch_w<T, 3, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        default: zsweep_launch_w<T, 4, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
+    }
+}
+
+// S (1 or 2) sweeps of level lv applied to u + P e_c (e_c = co's iterate `ec`): the trilinear correction is folded into the
+// pass, u itself is not modified.  Returns false (nothing launched) when the level's tiles are not full rows.
+bool launch_zsweep_prolong(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, const Level& co, const void* ec,
+                           const int* done)
+{
+    if (co.sx * 2 != lv.sx) return false;
+    if (c->es == 8) {
+        const ZCfg z = zcfg<double>(c, lv, S, false, true);
+        if (!z.ok) return false;
+        count_launch(c);
+        if (rhs) { if (S == 2) zsweep_launch_pro<double, 2, true>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<double, 1, true>(c, lv, z, u, rhs, out, done, ec, co.sp); }
+        else { if (S == 2) zsweep_launch_pro<double, 2, false>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<double, 1, false>(c, lv, z, u, rhs, out, done, ec, co.sp); }
+    } else {
+        const ZCfg z = zcfg<float>(c, lv, S, false, true);
+        if (!z.ok) return false;
+        count_launch(c);
+        if (rhs) { if (S == 2) zsweep_launch_pro<float, 2, true>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<float, 1, true>(c, lv, z, u, rhs, out, done, ec, co.sp); }
+        else { if (S == 2) zsweep_launch_pro<float, 2, false>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<float, 1, false>(c, lv, z, u, rhs, out, done, ec, co.sp); }
+    }
+    return true;
 }
 
 bool zsweep_ok(const mhs_ctx* c, const Level& lv)

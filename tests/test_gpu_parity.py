@@ -52,7 +52,8 @@ WORKLOADS = {
 }
 # fast: the default launch shapes;  big: the big-level (HBM-bound) kernels forced onto these small grids;
 # unfused: tuned kernels without temporal blocking / separable restriction;  reference: the paper's kernel design
-VARIANTS = {"fast": 0, "big": 8, "unfused": 4 | 8, "reference": 1}
+# big_sep: as big, with the prolongation kept a pass of its own (by default it is folded into the first post-smoothing pass)
+VARIANTS = {"fast": 0, "big": 8, "big_sep": 8 | 16, "unfused": 4 | 8, "reference": 1}
 
 
 def flags_of(B, variant):
