@@ -74,6 +74,7 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
                                         can handle, whatever its size; for parity tests on small grids     */
 #define MHS_FLAG_SEPARATE_PROLONG  16 /* keep the prolongation a pass of its own instead of folding it into the
                                         first post-smoothing pass of the big levels; for A/B tests              */
+#define MHS_FLAG_NO_PDL            32 /* launch every kernel fully serialised (no programmatic dependent launch)   */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 

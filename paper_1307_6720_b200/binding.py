@@ -23,6 +23,7 @@ MHS_FLAG_SYNC_EACH_CYCLE = 2
 MHS_FLAG_UNFUSED_KERNELS = 4
 MHS_FLAG_BIG_LEVEL_KERNELS = 8
 MHS_FLAG_SEPARATE_PROLONG = 16
+MHS_FLAG_NO_PDL = 32
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8
 (MHS_OK, MHS_ERR_INVALID_ARG, MHS_ERR_GRID, MHS_ERR_NOT_ELLIPTIC, MHS_ERR_INDEFINITE, MHS_ERR_STATE,

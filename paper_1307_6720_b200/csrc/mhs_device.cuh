@@ -25,6 +25,17 @@ __device__ __forceinline__ T apply_L(const LP<T>& p, const T* __restrict__ u, lo
     return lu;
 }
 
+// Programmatic dependent launch (PDL): the kernels of a cycle are a chain of small dependent launches, and on the levels
+// that live in the L2 launch latency is most of their time.  Every kernel starts with pdl_enter(): it lets the NEXT kernel
+// of the stream be scheduled as soon as all blocks of this one are running (its blocks then sit in their own pdl_enter),
+// and it waits until the PREVIOUS kernel has completed and its writes are visible.  Nothing that depends on earlier
+// kernels (not even the `done` flag) may be touched before it.  Without the launch attribute both are no-ops.
+__device__ __forceinline__ void pdl_enter()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll

@@ -91,6 +91,19 @@ namespace mhs {
 
 inline void count_launch(mhs_ctx* c) { c->prof.launches[c->cur_kc] += 1; }
 
+// Launch with the programmatic-stream-serialization attribute (PDL, see pdl_enter() in mhs_device.cuh).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(const mhs_ctx* c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = (c->opt.flags & MHS_FLAG_NO_PDL) ? 0 : 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ---- launchers of the reference kernels (mhs_kernels_ref.cu) --------------------------------
 // `done` (may be NULL) points at Ctl::done: when set, the kernel returns without doing anything.
 void launch_smooth_ref(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done);

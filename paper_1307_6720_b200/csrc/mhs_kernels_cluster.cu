@@ -420,6 +420,7 @@ __device__ void ph_prolong(const GLevelP<T>& L, T* __restrict__ u, const T* __re
 template <typename T, bool D3>
 __global__ void __launch_bounds__(CL_THREADS, 1) k_cluster(const __grid_constant__ ClusterP<T> P, const int* __restrict__ done)
 {
+    pdl_enter();
     if (P.mode != 2 && done && *done) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T* S = reinterpret_cast<T*>(smem_raw);
@@ -600,10 +601,12 @@ static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, 
     cfg.blockDim = dim3(CL_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = c->stream;
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = (unsigned)ncta; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // PDL, see pdl_enter() in mhs_device.cuh
+    at[1].val.programmaticStreamSerializationAllowed = (c->opt.flags & MHS_FLAG_NO_PDL) ? 0 : 1;
+    cfg.attrs = at; cfg.numAttrs = 2;
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, P, done);
     if (e != cudaSuccess || getenv("MHS_DEBUG"))
         fprintf(stderr, "[mhs] k_cluster<%s,%dD> mode %d levels [%d,%d) tail [%d,%d) cluster %d smem %zu: %s\n", sizeof(T) == 8 ? "f64" : "f32",

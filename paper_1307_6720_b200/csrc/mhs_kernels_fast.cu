@@ -71,6 +71,7 @@ __global__ void __launch_bounds__(128) k_smooth_z(LP<T> p, const T* __restrict__
                                                    const int* __restrict__ done)
 {
     static_assert(!ZERO2 || (HAS_RHS && STORE && !NORM), "ZERO2 is a plain sweep with a right-hand side");
+    pdl_enter();
     if (done && *done) return;
     if (ZERO2) u = rhs;
     constexpr int V = VN<T>::N;
@@ -153,6 +154,7 @@ __global__ void __launch_bounds__(128) k_smooth_z(LP<T> p, const T* __restrict__
 template <typename T>
 __global__ void __launch_bounds__(256) k_scale_rhs(LP<T> p, const T* __restrict__ rhs, T* __restrict__ u, const int* __restrict__ done)
 {
+    pdl_enter();
     if (done && *done) return;
     constexpr int V = VN<T>::N;
     const long long nv = p.sp / V;
@@ -178,6 +180,7 @@ __global__ void __launch_bounds__(128) k_resid_restrict_z(LP<T> p, const T* __re
                                                            long long csp, int cnz, T* __restrict__ rc, int Kchunk, int nzc, int reverse,
                                                            const int* __restrict__ done)
 {
+    pdl_enter();
     if (done && *done) return;
     constexpr int V = VN<T>::N;
     constexpr int VC = V / 2;
@@ -275,6 +278,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) k_prolong_v(int sx, int sy, long long sp, T* __restrict__ u, int csx, long long csp,
                                                     const T* __restrict__ ec, int reverse, int nzi, const int* __restrict__ done)
 {
+    pdl_enter();
     if (done && *done) return;
     constexpr int V = VN<T>::N;
     constexpr int VC = V / 2;
@@ -365,7 +369,7 @@ static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const vo
     const int kchunk = (planes + nzc - 1) / nzc;
     const int nzc2 = (planes + kchunk - 1) / kchunk;
     dim3 grid((unsigned)xb, (unsigned)nzc2);
-    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, lv), (const T*)u, (const T*)rhs, (T*)out, kchunk, nzc2, reverse, c->partial, done);
+    launch_pdl(c, kern, grid, dim3(128), 0, lp_of<T>(c, lv), (const T*)u, (const T*)rhs, (T*)out, kchunk, nzc2, reverse, c->partial, done);
     return xb * nzc2;
 }
 
@@ -430,7 +434,7 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
     const int Kchunk = (planes + nzc - 1) / nzc;
     const int nzc2 = (planes + Kchunk - 1) / Kchunk;
     dim3 grid((unsigned)xb, (unsigned)nzc2);
-    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sp, co.nz, (T*)rc, Kchunk, nzc2, reverse, done);
+    launch_pdl(c, kern, grid, dim3(128), 0, lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sp, co.nz, (T*)rc, Kchunk, nzc2, reverse, done);
 }
 
 void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
@@ -458,9 +462,9 @@ void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, cons
     const int V = c->es == 8 ? 2 : 4;
     dim3 grid((unsigned)((f.sp / V + 255) / 256), (unsigned)(f.nz - 2));
     if (c->es == 8)
-        k_prolong_v<double><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (double*)u, co.sx, co.sp, (const double*)ec, reverse, f.nz - 2, done);
+        launch_pdl(c, k_prolong_v<double>, grid, dim3(256), 0, f.sx, f.sy, f.sp, (double*)u, co.sx, co.sp, (const double*)ec, reverse, f.nz - 2, done);
     else
-        k_prolong_v<float><<<grid, 256, 0, c->stream>>>(f.sx, f.sy, f.sp, (float*)u, co.sx, co.sp, (const float*)ec, reverse, f.nz - 2, done);
+        launch_pdl(c, k_prolong_v<float>, grid, dim3(256), 0, f.sx, f.sy, f.sp, (float*)u, co.sx, co.sp, (const float*)ec, reverse, f.nz - 2, done);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -479,6 +483,7 @@ __global__ void __launch_bounds__(128) k_resid_restrict_sep(LP<T> p, const T* __
                                                             long long csp, int cnz, T* __restrict__ rc, int Kchunk, int reverse,
                                                             const int* __restrict__ done)
 {
+    pdl_enter();
     if (done && *done) return;
     constexpr int V = VN<T>::N;
     constexpr int VC = V / 2;
@@ -627,7 +632,7 @@ static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, cons
     const int Kchunk = (planes + nzc - 1) / nzc;
     nzc = (planes + Kchunk - 1) / Kchunk;
     dim3 grid((unsigned)xb, (unsigned)nzc);
-    kern<<<grid, 128, 0, c->stream>>>(lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sy, co.sp, co.nz, (T*)rc, Kchunk, reverse, done);
+    launch_pdl(c, kern, grid, dim3(128), 0, lp_of<T>(c, f), (const T*)u, (const T*)rhs, co.sx, co.sy, co.sp, co.nz, (T*)rc, Kchunk, reverse, done);
 }
 
 void launch_resid_restrict_sep(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)

@@ -135,6 +135,7 @@ __global__ void __launch_bounds__(256) k_resnorm_partial_ref(LP<T> p, const T* _
 // Deterministic final reduction + stop rule (C10; stop_rule in mhs_device.cuh): one block, fixed summation order.
 __global__ void __launch_bounds__(1024) k_norm_final(const double* __restrict__ partial, long long n, Ctl* ctl, int mode)
 {
+    pdl_enter();
     if (mode == 1 && ctl->done) return;
     double v = 0.0;
     for (long long q = threadIdx.x; q < n; q += 1024) v += partial[q];
@@ -329,7 +330,7 @@ long long resnorm_partial_capacity(const Level& lv)
 void launch_norm_final(mhs_ctx* c, long long n, int mode)
 {
     count_launch(c);
-    k_norm_final<<<1, 1024, 0, c->stream>>>(c->partial, n, c->ctl, mode);
+    launch_pdl(c, k_norm_final, dim3(1), dim3(1024), 0, (const double*)c->partial, n, c->ctl, mode);
 }
 
 void launch_pack(mhs_ctx* c, const Level& lv, const void* dense, void* dst, bool keep_bottom, bool negate)

@@ -562,6 +562,7 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
     static_assert(!ZERO || HAS_RHS, "a zero iterate with a zero right-hand side stays zero");
     static_assert(!PRO || (!ZERO && !NORM), "the prolongation-fused pass is a post-smoothing pass");
     constexpr int NIN = PRO ? 3 : ZNIN;
+    pdl_enter();
     if (done && *done) return;
     constexpr int V = ZV<T>::N;
     constexpr int NCO = ZV<T>::NCO;
@@ -793,7 +794,7 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
     p.ec = (const T*)ec; p.csp = csp;
-    kern<<<z.ctas, WXT * ZWY * 32, z.smem, c->stream>>>(p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
+    launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZWY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (getenv("MHS_DEBUG")) {
         cudaError_t e = cudaPeekAtLastError();
         fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",

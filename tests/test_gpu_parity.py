@@ -356,6 +356,32 @@ def test_boundary_only_context(B, orc, dtype):
             assert e.value.status == B.MHS_ERR_STATE
 
 
+@pytest.mark.parametrize("name", ["cfg0_33", "cfg1_65", "cfg1_129", "ragged_25x49x13", "cfg4_129x129x33"])
+def test_dependent_launch_is_invisible(B, name):
+    """Kernels are launched with programmatic dependent launch (the next kernel is scheduled while the previous one runs
+    and waits in griddepcontrol.wait).  Every kernel is deterministic, so the whole solve must be BITWISE the same with
+    and without it, every time: a read of stale data anywhere would show here."""
+    w = WORKLOADS[name]()
+    dt = torch.float64 if w.dtype == "f64" else torch.float32
+    ref = None
+    for rep in range(4):
+        for flags in (B.MHS_FLAG_NO_PDL, 0, B.MHS_FLAG_BIG_LEVEL_KERNELS, B.MHS_FLAG_BIG_LEVEL_KERNELS | B.MHS_FLAG_NO_PDL):
+            with B.Solver.from_workload(w, flags=flags) as S:
+                ib = S.solve_boundary(dev(w.Bz0, dt))
+                ii = S.solve_interior(w.tol, w.max_cycles)
+                P = S.get_potential().clone()
+                Bf, p, rho = S.fields()
+            key = bool(flags & B.MHS_FLAG_BIG_LEVEL_KERNELS)
+            if ref is None:
+                ref = {}
+            if key not in ref:
+                ref[key] = (P, Bf.clone(), ii["cycles"])
+            else:
+                assert ii["cycles"] == ref[key][2]
+                assert torch.equal(P, ref[key][0]), (name, rep, flags)
+                assert torch.equal(Bf, ref[key][1]), (name, rep, flags)
+
+
 def test_full_size_per_iterate_parity(B, orc):
     """BASELINE configs[2] at FULL size (257^3 fp64) in the launch configuration bench.py times (default flags:
     temporally blocked finest level, fine-grained mid levels, shared-memory tail): the first V-cycle iterates are
