@@ -35,13 +35,16 @@
 namespace mhs {
 
 template <typename T> struct ZV;
-template <> struct ZV<double> { static constexpr int N = 2; static constexpr int NCO = 6; };
-template <> struct ZV<float> { static constexpr int N = 4; static constexpr int NCO = 4; };
+// N: elements of a 128-bit vector; NCO: coefficients per plane record; R: rows of a thread's patch; WY: warps of a tile
+// along y (a tile has WY*R = 16 patch rows).  fp64: 8 rows x 256 threads x <= 255 registers ("few fat threads": measured
+// 62.5 us per 2-sweep pass at 257^3 against 68 us for 4 rows x 512 threads); fp32, with half the registers per value and the
+// longer difference-form update, is faster the other way round (1025^2 x 257: 632 us against 900 us per pass).
+template <> struct ZV<double> { static constexpr int N = 2, NCO = 6, R = 8, WY = 2; };
+template <> struct ZV<float> { static constexpr int N = 4, NCO = 4, R = 4, WY = 4; };
 
-constexpr int ZR = 8;     // rows of a thread's patch
-constexpr int ZWY = 2;    // warps of a tile along y: a tile has ZWY*ZR patch rows
 // Tile geometry is a compile-time function of WXT (warps along x), so that every shared-memory stride is an immediate:
 template <typename T, int WXT> struct ZG {
+    static constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY;
     static constexpr int TC = WXT * 32 * ZV<T>::N;          // tile columns
     static constexpr int INP = (ZWY * ZR + 2) * TC;         // elements of one ring slot / exchange plane
     // prolongation-fused variant (full-row tiles only): the coarse rows under the ZWY*ZR+2 fine rows of a tile
@@ -62,7 +65,7 @@ struct __align__(16) ZVec {
 
 template <typename T>
 struct Patch {
-    ZVec<T> r[ZR];
+    ZVec<T> r[ZV<T>::R];
 };
 
 template <typename T>
@@ -267,6 +270,7 @@ struct ZCtx {
 template <typename T, int WXT, int NIN>
 __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int nload, int k)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     const int slot = ring_slot<NIN>(nload);
     constexpr int TCc = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
     T* dst = IN + (size_t)slot * INP;
@@ -360,6 +364,7 @@ __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* t
 template <typename T, int WXT, int JP>
 __device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, uint32_t c0a, uint32_t c1a)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N, VC = V / 2;
     constexpr uint32_t ES = sizeof(T);
     constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES, crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
@@ -389,6 +394,7 @@ __device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, 
 template <typename T, int WXT, int NIN>
 __device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int t, int slot)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N, VC = V / 2;
     constexpr uint32_t ES = sizeof(T);
     constexpr int TC = ZG<T, WXT>::TC, NR = ZWY * ZR;
@@ -407,7 +413,7 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int 
     const int nvr = TC / V;
     const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
     const int jh = which ? z.jt + NR : z.jt - 1;
-    if (jh >= 1 && jh < p.sy) {
+    if (which < 2 && jh >= 1 && jh < p.sy) {
         const uint32_t a = z.in_base + (uint32_t)slot * planeb + (uint32_t)(((which ? NR + 1 : 0) * TC + hv * V) * ES);
         const uint32_t co = (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)ES);
         const uint32_t dj = (jh & 1) ? crowb : 0u;      // J1 = J0 + (j odd)
@@ -430,6 +436,7 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int 
 template <typename T, int WXT, bool ZERO, bool PRO>
 __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int NIN = PRO ? 3 : ZNIN;
     if (!ZERO) {
         const int pos = z.zoff + z.t;
@@ -449,6 +456,7 @@ template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool P
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N;
     constexpr uint32_t ES = sizeof(T);
     constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES;
@@ -555,9 +563,10 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
 }
 
 template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
-__global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
+__global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
 {
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     static_assert(S == 1 || S == 2, "S sweeps per pass: 1 or 2");
     static_assert(!ZERO || HAS_RHS, "a zero iterate with a zero right-hand side stays zero");
     static_assert(!PRO || (!ZERO && !NORM), "the prolongation-fused pass is a post-smoothing pass");
@@ -717,7 +726,7 @@ __global__ void __launch_bounds__(WXT * ZWY * 32, 1) k_zsweep(const __grid_const
 // ------------------------------------------------------------------------------------------------
 struct ZCfg {
     bool ok = false;
-    int WX = 0, WY = ZWY, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
+    int WX = 0, WY = 0, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
     size_t smem = 0;
 };
 
@@ -726,6 +735,7 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro =
 {
     constexpr int V = ZV<T>::N;
     constexpr int NCO = ZV<T>::NCO;
+    constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY;
     ZCfg z;
     if (lv.dim != 3 || lv.coarsest || lv.nz < 5) return z;
     const int lane_cols = 32 * V;
@@ -794,7 +804,7 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
     p.ec = (const T*)ec; p.csp = csp;
-    launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZWY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
+    launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZV<T>::WY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (getenv("MHS_DEBUG")) {
         cudaError_t e = cudaPeekAtLastError();
         fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
