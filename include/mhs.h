@@ -156,6 +156,14 @@ mhs_status mhs_solve_interior(mhs_ctx *ctx, double tol, int max_cycles, mhs_solv
  * p, rho: N values each, N = nx*ny*nz.  Any of B, p, rho may be NULL (skipped). */
 mhs_status mhs_fields(mhs_ctx *ctx, void *B_device, void *p_device, void *rho_device);
 mhs_status mhs_fields_host(mhs_ctx *ctx, void *B_host, void *p_host, void *rho_host);
+/* The same without waiting for the copies: the fields are computed on the context's stream into the library's staging
+ * buffer and copied to the (pinned) host buffers on a separate copy stream; the call returns as soon as that is enqueued,
+ * so the next mhs_solve_* can run while the results of this one travel over PCIe.  The host buffers must not be read, and
+ * must stay valid, until mhs_host_sync() has returned.  A later mhs_fields_host* / mhs_get_potential_host first waits
+ * (on the device) for the pending copies, so one staging buffer serves any pipeline depth. */
+mhs_status mhs_fields_host_async(mhs_ctx *ctx, void *B_host, void *p_host, void *rho_host);
+/* Block until every copy enqueued by mhs_fields_host_async has landed in host memory. */
+mhs_status mhs_host_sync(mhs_ctx *ctx);
 
 /* Read / overwrite the current iterate P (N values, dense).  mhs_set_potential takes the interior
  * and bottom-plane interior values; side/top/bottom-edge values of the input are ignored (they
@@ -169,6 +177,10 @@ const char *mhs_status_string(mhs_status s);
 
 /* ---- instrumentation ------------------------------------------------------------------------ */
 mhs_status mhs_get_profile(mhs_ctx *ctx, mhs_profile *out); /* synchronises the stream             */
+/* Change mhs_options.profile (0: launch counts only; 1: CUDA events around the finest-level smoothing / prolongation
+ * launches; 2: around every kernel class).  Event records between kernels undo the overlap of dependent launches and of
+ * the copy stream, so timing runs that are not about kernel shares should use 0. */
+mhs_status mhs_set_profiling(mhs_ctx *ctx, int level);
 mhs_status mhs_reset_profile(mhs_ctx *ctx);
 const char *mhs_kernel_class_name(int kernel_class);
 

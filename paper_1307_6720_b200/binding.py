@@ -31,9 +31,9 @@ MHS_KC_COUNT = 8
 
 EXPORTS = [
     "mhs_default_options", "mhs_create", "mhs_destroy", "mhs_solve_boundary", "mhs_solve_boundary_host",
-    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_get_potential", "mhs_get_potential_host",
+    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_get_potential", "mhs_get_potential_host",
     "mhs_set_potential", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
-    "mhs_kernel_class_name", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
+    "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
 ]
 
@@ -95,8 +95,9 @@ def lib():
         for n in ("mhs_solve_boundary", "mhs_solve_boundary_host"):
             getattr(L, n).argtypes = [vp, vp, C.POINTER(mhs_solve_info)]
         L.mhs_solve_interior.argtypes = [vp, dp, ip, C.POINTER(mhs_solve_info)]
-        for n in ("mhs_fields", "mhs_fields_host"):
+        for n in ("mhs_fields", "mhs_fields_host", "mhs_fields_host_async"):
             getattr(L, n).argtypes = [vp, vp, vp, vp]
+        L.mhs_host_sync.argtypes = [vp]
         for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential"):
             getattr(L, n).argtypes = [vp, vp]
         L.mhs_last_error.argtypes = [vp]
@@ -105,6 +106,7 @@ def lib():
         L.mhs_status_string.restype = C.c_char_p
         L.mhs_get_profile.argtypes = [vp, C.POINTER(mhs_profile)]
         L.mhs_reset_profile.argtypes = [vp]
+        L.mhs_set_profiling.argtypes = [vp, ip]
         L.mhs_kernel_class_name.argtypes = [ip]
         L.mhs_kernel_class_name.restype = C.c_char_p
         L.mhs_num_levels.argtypes = [vp, ip]
@@ -214,9 +216,13 @@ def mhs_solve_interior(h, tol, max_cycles):
     return _info(i, st)
 
 
-def mhs_fields(h, B, p, rho, dtype, N, host=False):
+def mhs_host_sync(h):
+    _check(h, lib().mhs_host_sync(h))
+
+
+def mhs_fields(h, B, p, rho, dtype, N, host=False, wait=True):
     dev = "cpu" if host else "cuda"
-    fn = lib().mhs_fields_host if host else lib().mhs_fields
+    fn = (lib().mhs_fields_host if wait else lib().mhs_fields_host_async) if host else lib().mhs_fields
     _check(h, fn(h, _dptr(B, dtype, 3 * N, dev), _dptr(p, dtype, N, dev), _dptr(rho, dtype, N, dev)))
 
 
@@ -284,7 +290,10 @@ class Solver:
     def solve_interior(self, tol=1e-10, max_cycles=100):
         return mhs_solve_interior(self.h, tol, max_cycles)
 
-    def fields(self, B=None, p=None, rho=None, want=("B", "p", "rho"), host=False):
+    def host_sync(self):
+        mhs_host_sync(self.h)
+
+    def fields(self, B=None, p=None, rho=None, want=("B", "p", "rho"), host=False, wait=True):
         dev = "cpu" if host else "cuda"
         mk = lambda n: torch.empty(n, dtype=self.dtype, device=dev, pin_memory=host)
         if B is None and "B" in want:
@@ -293,7 +302,7 @@ class Solver:
             p = mk(self.N)
         if rho is None and "rho" in want:
             rho = mk(self.N)
-        mhs_fields(self.h, B, p, rho, self.dtype, self.N, host=host)
+        mhs_fields(self.h, B, p, rho, self.dtype, self.N, host=host, wait=wait)
         shp = (self.nz, self.ny, self.nx)
         return (None if B is None else B.view(3, *shp), None if p is None else p.view(shp),
                 None if rho is None else rho.view(shp))
@@ -312,6 +321,9 @@ class Solver:
 
     def reset_profile(self):
         mhs_reset_profile(self.h)
+
+    def set_profiling(self, level):
+        _check(self.h, lib().mhs_set_profiling(self.h, int(level)))
 
     # -- operator-level access (tests / micro-benchmarks)
     def num_levels(self, dim=3):

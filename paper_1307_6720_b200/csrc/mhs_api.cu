@@ -6,7 +6,7 @@
 #include <cstring>
 #include <new>
 
-#include "mhs_internal.h"
+#include "mhs_device.cuh"
 
 using namespace mhs;
 
@@ -20,6 +20,30 @@ namespace {
             return e_ == cudaErrorMemoryAllocation ? MHS_ERR_OOM : MHS_ERR_CUDA;                         \
         }                                                                                                \
     } while (0)
+
+// The control block goes back to the host by STORES into mapped pinned memory, not by a DMA copy: a copy would queue on
+// the device->host copy engine behind the 679 MB of field results that mhs_fields_host_async may have in flight, and the
+// solve loop of the next step would stall on it.
+__global__ void k_ctl_to_host(const Ctl* __restrict__ ctl, Ctl* host)
+{
+    pdl_enter();
+    const int n = (int)(sizeof(Ctl) / sizeof(int));
+    const int* s = reinterpret_cast<const int*>(ctl);
+    int* d = reinterpret_cast<int*>(host);
+    for (int i = threadIdx.x; i < n; i += blockDim.x) d[i] = s[i];
+    __threadfence_system();
+}
+
+mhs_status read_ctl(mhs_ctx* ctx)
+{
+    launch_pdl(ctx, k_ctl_to_host, dim3(1), dim3(256), 0, (const Ctl*)ctx->ctl, ctx->ctl_host);
+    cudaError_t e_ = cudaStreamSynchronize(ctx->stream);
+    if (e_ != cudaSuccess) {
+        ctx->err = std::string("cudaStreamSynchronize: ") + cudaGetErrorString(e_);
+        return MHS_ERR_CUDA;
+    }
+    return MHS_OK;
+}
 
 mhs_status fail(mhs_ctx* ctx, mhs_status s, const std::string& msg)
 {
@@ -449,8 +473,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
             Scope sc(ctx, kc_for(l0, 0, 0));
             launch_cluster(ctx, Ls, 0, 2, nullptr);
         }
-        CK(cudaMemcpyAsync(h, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
-        CK(cudaStreamSynchronize(ctx->stream));
+        { mhs_status rs = read_ctl(ctx); if (rs) return rs; }
         drain_events(ctx);
         CK(cudaGetLastError());
         if ((h->cycles * (ctx->opt.n_pre + ctx->opt.n_post)) & 1) std::swap(l0.u, l0.tmp);
@@ -490,8 +513,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
             norm_final(ctx, l0, 0, np, 1);
             trailing = true;
         }
-        CK(cudaMemcpyAsync(h, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
-        CK(cudaStreamSynchronize(ctx->stream));
+        { mhs_status rs = read_ctl(ctx); if (rs) return rs; }
         if (h->done || trailing) break;
     }
     drain_events(ctx);
@@ -504,9 +526,17 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
     return finish_cycles(ctx, tol, info);
 }
 
+// pending host copies (mhs_fields_host_async) read the staging buffer: later work on the main stream that overwrites it waits
+mhs_status stage_fence(mhs_ctx* ctx)
+{
+    if (ctx->copy_pending) CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_copied, 0));
+    return MHS_OK;
+}
+
 mhs_status ensure_stage(mhs_ctx* ctx, size_t bytes)
 {
     if (ctx->stage_bytes >= bytes) return MHS_OK;
+    if (ctx->copy_pending) { CK(cudaEventSynchronize(ctx->ev_copied)); ctx->copy_pending = false; }
     if (ctx->stage) cudaFree(ctx->stage);
     ctx->stage = nullptr; ctx->stage_bytes = 0;
     CK(cudaMalloc(&ctx->stage, bytes));
@@ -649,8 +679,8 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
     CK(cudaMalloc((void**)&ctx->ctl, sizeof(Ctl)));
     CK(cudaMemset(ctx->ctl, 0, sizeof(Ctl)));
-    CK(cudaMallocHost((void**)&ctx->ctl_host, sizeof(Ctl)));
-    if ((st = ensure_stage(ctx, (size_t)grid->nx * grid->ny * ctx->es))) return st;
+    CK(cudaHostAlloc((void**)&ctx->ctl_host, sizeof(Ctl), cudaHostAllocMapped));   // (unified addressing: usable on the device as is)
+    CK(cudaMalloc(&ctx->bz_stage, (size_t)grid->nx * grid->ny * ctx->es));
     CK(cudaDeviceSynchronize());
     return MHS_OK;
 }
@@ -669,7 +699,11 @@ void mhs_destroy(mhs_ctx* ctx)
     if (ctx->partial) cudaFree(ctx->partial);
     if (ctx->ctl) cudaFree(ctx->ctl);
     if (ctx->ctl_host) cudaFreeHost(ctx->ctl_host);
+    if (ctx->copy_stream) { cudaStreamSynchronize(ctx->copy_stream); cudaStreamDestroy(ctx->copy_stream); }
+    if (ctx->ev_fields) cudaEventDestroy(ctx->ev_fields);
+    if (ctx->ev_copied) cudaEventDestroy(ctx->ev_copied);
     if (ctx->stage) cudaFree(ctx->stage);
+    if (ctx->bz_stage) cudaFree(ctx->bz_stage);
     for (const Ev& e : ctx->ev_pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
@@ -713,11 +747,10 @@ mhs_status mhs_solve_boundary_host(mhs_ctx* ctx, const void* Bz0_host, mhs_solve
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (!Bz0_host) return fail(ctx, MHS_ERR_INVALID_ARG, "Bz0 is NULL");
+    // (a buffer of its own: the big staging buffer may still be feeding the host copies of the previous step's fields)
     const size_t bytes = (size_t)ctx->grid.nx * ctx->grid.ny * ctx->es;
-    mhs_status st = ensure_stage(ctx, bytes);
-    if (st) return st;
-    CK(cudaMemcpyAsync(ctx->stage, Bz0_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
-    return mhs_solve_boundary(ctx, ctx->stage, info);
+    CK(cudaMemcpyAsync(ctx->bz_stage, Bz0_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    return mhs_solve_boundary(ctx, ctx->bz_stage, info);
 }
 
 mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solve_info* info)
@@ -754,6 +787,7 @@ mhs_status mhs_get_potential_host(mhs_ctx* ctx, void* P_host)
     const size_t bytes = (size_t)ctx->L3[0].npts() * ctx->es;
     mhs_status st = ensure_stage(ctx, bytes);
     if (st) return st;
+    if ((st = stage_fence(ctx))) return st;
     if ((st = mhs_get_potential(ctx, ctx->stage))) return st;
     CK(cudaMemcpyAsync(P_host, ctx->stage, bytes, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
@@ -792,21 +826,47 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
     return MHS_OK;
 }
 
-mhs_status mhs_fields_host(mhs_ctx* ctx, void* B, void* p, void* rho)
+mhs_status mhs_fields_host_async(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
     const size_t nb = (size_t)ctx->L3[0].npts() * ctx->es;
     mhs_status st = ensure_stage(ctx, 5 * nb);
     if (st) return st;
+    if (!ctx->copy_stream) {
+        CK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&ctx->ev_fields, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&ctx->ev_copied, cudaEventDisableTiming));
+    }
+    if ((st = stage_fence(ctx))) return st;     // the previous results must have left the staging buffer
     char* s = (char*)ctx->stage;
     if ((st = mhs_fields(ctx, B ? s : nullptr, p ? s + 3 * nb : nullptr, rho ? s + 4 * nb : nullptr))) return st;
-    if (B) CK(cudaMemcpyAsync(B, s, 3 * nb, cudaMemcpyDeviceToHost, ctx->stream));
-    if (p) CK(cudaMemcpyAsync(p, s + 3 * nb, nb, cudaMemcpyDeviceToHost, ctx->stream));
-    if (rho) CK(cudaMemcpyAsync(rho, s + 4 * nb, nb, cudaMemcpyDeviceToHost, ctx->stream));
-    CK(cudaStreamSynchronize(ctx->stream));
+    CK(cudaEventRecord(ctx->ev_fields, ctx->stream));
+    CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_fields, 0));
+    if (B) CK(cudaMemcpyAsync(B, s, 3 * nb, cudaMemcpyDeviceToHost, ctx->copy_stream));
+    if (p) CK(cudaMemcpyAsync(p, s + 3 * nb, nb, cudaMemcpyDeviceToHost, ctx->copy_stream));
+    if (rho) CK(cudaMemcpyAsync(rho, s + 4 * nb, nb, cudaMemcpyDeviceToHost, ctx->copy_stream));
+    CK(cudaEventRecord(ctx->ev_copied, ctx->copy_stream));
+    ctx->copy_pending = true;
+    return MHS_OK;
+}
+
+mhs_status mhs_host_sync(mhs_ctx* ctx)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->copy_pending) {
+        CK(cudaEventSynchronize(ctx->ev_copied));
+        ctx->copy_pending = false;
+    }
     drain_events(ctx);
     return MHS_OK;
+}
+
+mhs_status mhs_fields_host(mhs_ctx* ctx, void* B, void* p, void* rho)
+{
+    mhs_status st = mhs_fields_host_async(ctx, B, p, rho);
+    if (st) return st;
+    return mhs_host_sync(ctx);
 }
 
 mhs_status mhs_get_profile(mhs_ctx* ctx, mhs_profile* out)
@@ -815,6 +875,15 @@ mhs_status mhs_get_profile(mhs_ctx* ctx, mhs_profile* out)
     CK(cudaStreamSynchronize(ctx->stream));
     drain_events(ctx);
     *out = ctx->prof;
+    return MHS_OK;
+}
+
+mhs_status mhs_set_profiling(mhs_ctx* ctx, int level)
+{
+    if (!ctx || level < 0 || level > 2) return MHS_ERR_INVALID_ARG;
+    CK(cudaStreamSynchronize(ctx->stream));
+    drain_events(ctx);
+    ctx->opt.profile = level;
     return MHS_OK;
 }
 
@@ -966,8 +1035,7 @@ mhs_status mhs_op_resnorm(mhs_ctx* ctx, int dim, int level, double* out_host)
         const long long np = resnorm_partials(ctx, *Ls, level, nullptr);
         norm_final(ctx, (*Ls)[level], level, np, 2);
     }
-    CK(cudaMemcpyAsync(ctx->ctl_host, ctx->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, ctx->stream));
-    CK(cudaStreamSynchronize(ctx->stream));
+    { mhs_status rs = read_ctl(ctx); if (rs) return rs; }
     drain_events(ctx);
     *out_host = ctx->ctl_host->r_last;
     return MHS_OK;

@@ -73,6 +73,10 @@ struct mhs_ctx {
     long long npartial = 0;
     void* stage = nullptr;         // device staging for host-pointer entry points (lazy)
     size_t stage_bytes = 0;
+    void* bz_stage = nullptr;      // device copy of a host magnetogram (mhs_solve_boundary_host)
+    cudaStream_t copy_stream = nullptr;                  // device -> host copies of mhs_fields_host_async
+    cudaEvent_t ev_fields = nullptr, ev_copied = nullptr;
+    bool copy_pending = false;
     bool have_boundary = false, have_r0 = false;
     double r0_interior = 0;
     mhs_profile prof{};

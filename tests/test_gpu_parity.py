@@ -274,6 +274,36 @@ def test_full_pipeline_host_buffers(B, orc):
 
 
 # ------------------------------------------------------------------ edge cases ---------------
+def test_pipelined_host_fields(B):
+    """mhs_fields_host_async + mhs_host_sync: results of consecutive steps land in alternating host buffers while the
+    next solve runs; they must equal the blocking call's, bit for bit."""
+    w = inputs.config(1, shrink=2)
+    N = w.npoints
+    mk = lambda: (torch.empty(3 * N, dtype=torch.float64).pin_memory(), torch.empty(N, dtype=torch.float64).pin_memory(),
+                  torch.empty(N, dtype=torch.float64).pin_memory())
+    bufs = [mk(), mk()]
+    ref = mk()
+    bz = [torch.as_tensor(w.Bz0 * s, dtype=torch.float64).contiguous().pin_memory() for s in (1.0, -0.5, 2.0)]
+    with B.Solver.from_workload(w) as S:
+        refs = []
+        for b in bz:
+            S.solve_boundary(b); S.solve_interior(w.tol, w.max_cycles)
+            S.fields(*ref, host=True)
+            refs.append([t.clone() for t in ref])
+        got = []
+        for k, b in enumerate(bz):
+            S.solve_boundary(b); S.solve_interior(w.tol, w.max_cycles)
+            if k >= 1:                      # the buffers of step k-1 are read only after a sync
+                S.host_sync()
+                got.append([t.clone() for t in bufs[(k - 1) % 2]])
+            S.fields(*bufs[k % 2], host=True, wait=False)
+        S.host_sync()
+        got.append([t.clone() for t in bufs[(len(bz) - 1) % 2]])
+        for r, g in zip(refs, got):
+            for a, c in zip(r, g):
+                assert torch.equal(a, c)
+
+
 def test_edge_cases(B, orc):
     # zero magnetogram: r0 = 0, one cycle, P stays 0, fields give the background
     w = inputs.config(0)
