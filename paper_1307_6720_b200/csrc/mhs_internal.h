@@ -95,6 +95,15 @@ namespace mhs {
 
 inline void count_launch(mhs_ctx* c) { c->prof.launches[c->cur_kc] += 1; }
 
+// Kernels that live on the L1 (no dynamic shared memory) say so ONCE: with no stated preference a kernel launched after one
+// that had the SM configured for 220 KB of shared memory (k_zsweep, the cluster kernel's tail) inherits that split and runs
+// with a ~28 KB L1 -- measured: residual+restriction 44 -> 61 us, 25 us per zsweep/restriction pair.
+template <typename K>
+inline void prefer_l1(K kern)
+{
+    cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxL1);
+}
+
 // Launch with the programmatic-stream-serialization attribute (PDL, see pdl_enter() in mhs_device.cuh).
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(const mhs_ctx* c, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args)

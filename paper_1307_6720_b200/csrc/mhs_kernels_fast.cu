@@ -358,6 +358,7 @@ static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const vo
     auto kern = k_smooth_z<T, R, HAS_RHS, STORE, NORM, ZERO2>;
     static int slots = 0;
     if (!slots) {
+        prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
         slots = std::max(1, nb) * c->num_sms;
@@ -408,6 +409,8 @@ long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
 
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done)
 {
+    static bool once = false;
+    if (!once) { prefer_l1(k_scale_rhs<double>); prefer_l1(k_scale_rhs<float>); once = true; }
     count_launch(c);
     const int V = c->es == 8 ? 2 : 4;
     dim3 grid((unsigned)((lv.sp / V + 255) / 256), (unsigned)(lv.nz - 2));
@@ -422,6 +425,7 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
     auto kern = k_resid_restrict_z<T, R, HAS_RHS>;
     static int slots = 0;
     if (!slots) {
+        prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
         slots = std::max(1, nb) * c->num_sms;
@@ -458,6 +462,8 @@ void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const vo
 
 void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, const void* ec, int reverse, const int* done)
 {
+    static bool once = false;
+    if (!once) { prefer_l1(k_prolong_v<double>); prefer_l1(k_prolong_v<float>); once = true; }
     count_launch(c);
     const int V = c->es == 8 ? 2 : 4;
     dim3 grid((unsigned)((f.sp / V + 255) / 256), (unsigned)(f.nz - 2));
@@ -618,6 +624,7 @@ static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, cons
     auto kern = k_resid_restrict_sep<T, RC, HAS_RHS>;
     static int slots = 0;
     if (!slots) {
+        prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
         slots = std::max(1, nb) * c->num_sms;

@@ -229,6 +229,7 @@ static void fields_z_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void
     auto kern = k_fields_z<T>;
     static int slots = 0;
     if (!slots) {
+        prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 256, 0);
         slots = std::max(1, nb) * c->num_sms;
