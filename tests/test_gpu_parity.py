@@ -386,6 +386,59 @@ def test_boundary_only_context(B, orc, dtype):
             assert e.value.status == B.MHS_ERR_STATE
 
 
+@pytest.mark.parametrize("flags", [0, 8, 8 | 16, 4 | 8])
+@pytest.mark.parametrize("sweeps", [(2, 1), (1, 1), (3, 3), (1, 0), (0, 2), (3, 2), (1, 2)])
+def test_sweep_counts_on_the_big_level_kernels(B, orc, sweeps, flags):
+    """Odd / zero / three sweeps through the temporally blocked smoother (1- and 2-sweep passes, the zero-guess passes,
+    the prolongation-fused pass with 1 or 2 sweeps or -- n_post = 0 -- not at all) and the mid-level kernels."""
+    a, b = sweeps
+    w = inputs.config(1, shrink=2)
+    with B.Solver.from_workload(w, n_pre=a, n_post=b, flags=flags) as S:
+        S.solve_boundary(dev(w.Bz0, torch.float64))
+        P = host(S.get_potential())
+        c = 1.0 + w.f
+        for k in range(4):
+            S.solve_interior(0.0, 1)
+            P = orc.vcycle3(P, None, c, w.alpha, w.L, omega=w.omega, n_pre=a, n_post=b)
+            err = relmax(host(S.get_potential()), P)
+            assert err <= 1e-12, (sweeps, flags, k, err)
+
+
+def test_streams_and_concurrent_contexts(B, orc):
+    """Two contexts on two non-default streams, calls interleaved: each must give what it gives alone."""
+    w1, w2 = inputs.config(1, shrink=2), inputs.small(nx=33, ny=65, nz=17, L=(1.0, 2.0, 0.5), seed=5)
+    with B.Solver.from_workload(w1) as S:
+        S.solve_boundary(dev(w1.Bz0, torch.float64)); S.solve_interior(w1.tol, w1.max_cycles)
+        ref1 = S.get_potential().clone()
+    with B.Solver.from_workload(w2) as S:
+        S.solve_boundary(dev(w2.Bz0, torch.float64)); S.solve_interior(w2.tol, w2.max_cycles)
+        ref2 = S.get_potential().clone()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    b1, b2 = dev(w1.Bz0, torch.float64), dev(w2.Bz0, torch.float64)
+    torch.cuda.synchronize()
+    A = B.Solver.from_workload(w1, stream=s1)
+    C = B.Solver.from_workload(w2, stream=s2)
+    try:
+        A.solve_boundary(b1); C.solve_boundary(b2)
+        da = dc = False
+        for _ in range(40):
+            if not da:
+                da = A.solve_interior(w1.tol, 3)["converged"]
+            if not dc:
+                dc = C.solve_interior(w2.tol, 2)["converged"]
+            if da and dc:
+                break
+        assert da and dc
+        with torch.cuda.stream(s1):
+            Pa = A.get_potential()
+        with torch.cuda.stream(s2):
+            Pc = C.get_potential()
+        s1.synchronize(); s2.synchronize()
+        assert torch.equal(Pa, ref1) and torch.equal(Pc, ref2)
+    finally:
+        A.close(); C.close()
+
+
 @pytest.mark.parametrize("name", ["cfg0_33", "cfg1_65", "cfg1_129", "ragged_25x49x13", "cfg4_129x129x33"])
 def test_dependent_launch_is_invisible(B, name):
     """Kernels are launched with programmatic dependent launch (the next kernel is scheduled while the previous one runs
