@@ -299,7 +299,7 @@ template <typename T, int WXT, int NIN>
 __device__ __forceinline__ void c_request(const ZP<T>& p, ZCtx<T>& z, int kfine)
 {
     constexpr int CINP = ZG<T, WXT>::CINP, CSX = ZG<T, WXT>::CSX;
-    const int klast = min(kfine, p.nz - 2);
+    const int klast = min(min(kfine, z.kend_in), p.nz - 2);
     if (klast < 1) return;
     const int kneed = (klast + 1) >> 1;
     while (z.cnext <= kneed) {
@@ -347,7 +347,7 @@ __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* t
         const int k = z.t + NIN - 1;      // the slot of plane t-1 is free: request plane t+NIN-1 into it
         if (k <= z.kend_in) {
             if (threadIdx.x < 32) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, z.zoff + k, k);
-            if (PRO) c_request<T, WXT, NIN>(p, z, k);
+            if (PRO) c_request<T, WXT, NIN>(p, z, k + 1);   // (one plane ahead: the coarse plane is there when its fine plane lands)
         }
     }
     ++z.t;
@@ -657,13 +657,14 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
             ring += kend_in - kstart + 1;
             if (PRO) {
                 // coarse planes (kfirst >> 1) .. ((klast + 1) >> 1) serve the corrected fine planes kfirst .. klast
+                z.kend_in = kend_in;
                 z.jt = jt;
                 z.Jb = (jt - 1) >> 1;
                 const int kfirst = max(kstart, 1), klast = min(kend_in, p.nz - 2);
                 z.cnext = kfirst >> 1;
                 z.czoff = cring - z.cnext;
                 if (klast >= kfirst) cring += ((klast + 1) >> 1) - z.cnext + 1;
-                c_request<T, WXT, NIN>(p, z, kstart + n - 1);
+                c_request<T, WXT, NIN>(p, z, kstart + n);
             }
         }
         __syncthreads();   // coefficient table visible
