@@ -156,6 +156,12 @@ mhs_status mhs_solve_interior(mhs_ctx *ctx, double tol, int max_cycles, mhs_solv
  * p, rho: N values each, N = nx*ny*nz.  Any of B, p, rho may be NULL (skipped). */
 mhs_status mhs_fields(mhs_ctx *ctx, void *B_device, void *p_device, void *rho_device);
 mhs_status mhs_fields_host(mhs_ctx *ctx, void *B_host, void *p_host, void *rho_host);
+/* Diagnostics of the recovered field (the quantities of the paper's Figs 2, 4-7): |B| and the current
+ * density j = curl B / mu0 (eq 2) with |j|, by second-order central differences of B (one-sided second order
+ * in z on the bottom plane; j = 0 on the side and top boundary nodes, where B = 0 is imposed).
+ * B_device: the 3*N values mhs_fields wrote (Bx | By | Bz).  absB, absJ: N values; J: 3*N (jx | jy | jz); any of the three
+ * outputs may be NULL (skipped).  All device, dense, the context's dtype. */
+mhs_status mhs_diagnostics(mhs_ctx *ctx, const void *B_device, void *absB_device, void *J_device, void *absJ_device);
 /* The same without waiting for the copies: the fields are computed on the context's stream into the library's staging
  * buffer and copied to the (pinned) host buffers on a separate copy stream; the call returns as soon as that is enqueued,
  * so the next mhs_solve_* can run while the results of this one travel over PCIe.  The host buffers must not be read, and

@@ -89,6 +89,8 @@ def lib():
         L.orc_solve_boundary.restype = _i
         L.orc_solve_boundary.argtypes = g2 + [_p, _d, _i, _i, _i, _d, _i, _p, _p, _p, _i]
         L.orc_fields.argtypes = g3 + [_d, _p, _p, _p, _p, _d, _d, _p, _p, _p, _p, _p, _p]
+        L.orc_diagnostics.argtypes = g3 + [_d, _p, _p, _p, _p, _p, _p, _p, _p]
+        L.orc_diagnostics.restype = None
         _lib = L
     return _lib
 
@@ -303,4 +305,13 @@ def fields(P, f, alpha, Lxyz, p_b, rho_b, mu0=0.5, g=1.0, dfdz=None):
     out = [np.empty_like(P) for _ in range(5)]
     lib().orc_fields(nx, ny, nz, *Lxyz, alpha, _ptr(f), _ptr(dfdz), _ptr(p_b), _ptr(rho_b), mu0, g,
                      _ptr(P), *[_ptr(o) for o in out])
+    return tuple(out)
+
+
+def diagnostics(Bx, By, Bz, Lxyz, mu0=0.5):
+    """|B| and j = curl B / mu0 with |j| (eq 2; Figs 2, 4-7): returns (absB, jx, jy, jz, absJ)."""
+    Bx = _a(Bx); By = _a(By); Bz = _a(Bz)
+    nz, ny, nx = Bx.shape
+    out = [np.empty_like(Bx) for _ in range(5)]
+    lib().orc_diagnostics(nx, ny, nz, *Lxyz, mu0, _ptr(Bx), _ptr(By), _ptr(Bz), *[_ptr(o) for o in out])
     return tuple(out)

@@ -624,3 +624,35 @@ void orc_fields(int nx, int ny, int nz, double Lx, double Ly, double Lz, double 
             }
     }
 }
+
+/* ------------------------------------------------------------------------------------
+ * Diagnostics of a computed equilibrium (the quantities of the paper's Figs 2, 4-7,
+ * PAPER.md:164-196): |B| and the current density  j = curl B / mu0  (eq 2) with |j|.
+ * Second-order central differences of the B that orc_fields returns ("derivatives must be dealt with
+ * using finite differences"); on the bottom plane the z-derivatives are the one-sided second-order ones, as for B
+ * itself (C13); on the side and top boundary nodes, where B = 0 is imposed, j is set to 0.
+ * ---------------------------------------------------------------------------------- */
+void orc_diagnostics(int nx, int ny, int nz, double Lx, double Ly, double Lz, double mu0,
+                     const double *Bx, const double *By, const double *Bz,
+                     double *absB, double *jx, double *jy, double *jz, double *absJ)
+{
+    double hx = Lx / (nx - 1), hy = Ly / (ny - 1), hz = Lz / (nz - 1);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                size_t q = I3(i, j, k);
+                absB[q] = sqrt(Bx[q] * Bx[q] + By[q] * By[q] + Bz[q] * Bz[q]);
+                int wall = (i == 0 || i == nx - 1 || j == 0 || j == ny - 1 || k == nz - 1);
+                if (wall) { jx[q] = jy[q] = jz[q] = absJ[q] = 0.0; continue; }
+                double dyBz = (Bz[I3(i, j + 1, k)] - Bz[I3(i, j - 1, k)]) / (2.0 * hy);
+                double dxBz = (Bz[I3(i + 1, j, k)] - Bz[I3(i - 1, j, k)]) / (2.0 * hx);
+                double dxBy = (By[I3(i + 1, j, k)] - By[I3(i - 1, j, k)]) / (2.0 * hx);
+                double dyBx = (Bx[I3(i, j + 1, k)] - Bx[I3(i, j - 1, k)]) / (2.0 * hy);
+                double dzBy = dz_at(By, nx, ny, nz, i, j, k, hz);
+                double dzBx = dz_at(Bx, nx, ny, nz, i, j, k, hz);
+                double a = (dyBz - dzBy) / mu0, b = (dzBx - dxBz) / mu0, c = (dxBy - dyBx) / mu0;
+                jx[q] = a; jy[q] = b; jz[q] = c;
+                absJ[q] = sqrt(a * a + b * b + c * c);
+            }
+}

@@ -31,7 +31,7 @@ MHS_KC_COUNT = 8
 
 EXPORTS = [
     "mhs_default_options", "mhs_create", "mhs_destroy", "mhs_solve_boundary", "mhs_solve_boundary_host",
-    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_get_potential", "mhs_get_potential_host",
+    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_diagnostics", "mhs_get_potential", "mhs_get_potential_host",
     "mhs_set_potential", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
     "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
@@ -98,6 +98,7 @@ def lib():
         for n in ("mhs_fields", "mhs_fields_host", "mhs_fields_host_async"):
             getattr(L, n).argtypes = [vp, vp, vp, vp]
         L.mhs_host_sync.argtypes = [vp]
+        L.mhs_diagnostics.argtypes = [vp, vp, vp, vp, vp]
         for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential"):
             getattr(L, n).argtypes = [vp, vp]
         L.mhs_last_error.argtypes = [vp]
@@ -306,6 +307,17 @@ class Solver:
         shp = (self.nz, self.ny, self.nx)
         return (None if B is None else B.view(3, *shp), None if p is None else p.view(shp),
                 None if rho is None else rho.view(shp))
+
+    def diagnostics(self, B, want=("absB", "J", "absJ")):
+        """|B|, j = curl B / mu0, |j| of the field mhs_fields returned (B: 3N device tensor or its (3, nz, ny, nx) view)."""
+        mk = lambda n: torch.empty(n, dtype=self.dtype, device="cuda")
+        aB = mk(self.N) if "absB" in want else None
+        J = mk(3 * self.N) if "J" in want else None
+        aJ = mk(self.N) if "absJ" in want else None
+        _check(self.h, lib().mhs_diagnostics(self.h, _dptr(B.reshape(-1), self.dtype, 3 * self.N), _dptr(aB, self.dtype, self.N),
+                                             _dptr(J, self.dtype, 3 * self.N), _dptr(aJ, self.dtype, self.N)))
+        shp = (self.nz, self.ny, self.nx)
+        return (None if aB is None else aB.view(shp), None if J is None else J.view(3, *shp), None if aJ is None else aJ.view(shp))
 
     def get_potential(self, out=None):
         if out is None:

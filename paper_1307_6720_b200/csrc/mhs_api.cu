@@ -826,6 +826,19 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
     return MHS_OK;
 }
 
+mhs_status mhs_diagnostics(mhs_ctx* ctx, const void* B, void* absB, void* J, void* absJ)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
+    if (!B) return fail(ctx, MHS_ERR_INVALID_ARG, "B is NULL");
+    if (ctx->grid.nz < 3) return fail(ctx, MHS_ERR_GRID, "diagnostics need at least 3 planes");
+    if (!absB && !J && !absJ) return MHS_OK;
+    Scope sc(ctx, MHS_KC_FIELDS);
+    launch_diagnostics(ctx, ctx->L3[0], B, absB, J, absJ);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
 mhs_status mhs_fields_host_async(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;

@@ -135,6 +135,7 @@ void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void
 // ---- one-pass field recovery (mhs_kernels_fields.cu): planes 1 .. nz-2 ----
 bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
+void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ);
 
 // ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);

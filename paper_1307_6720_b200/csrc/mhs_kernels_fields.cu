@@ -254,4 +254,63 @@ void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* 
     else fields_z_t<float>(c, lv, P, B, p, rho);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Diagnostics (the quantities of the paper's Figs 2, 4-7): |B| and j = curl B / mu0 (eq 2,
+// PAPER.md:41) with |j|, from the dense B that mhs_fields returns.  Second-order central differences, one-sided second
+// order in z on the bottom plane (as for B itself, C13); j = 0 on the side and top boundary nodes, where B = 0 is imposed
+// (PAPER.md:134).  One thread per node: 3w read + up to 5w written per node, dense in and out.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) k_diagnostics(int nx, int ny, int nz, T i2hx, T i2hy, T i2hz, T imu0, const T* __restrict__ Bx,
+                                                      const T* __restrict__ By, const T* __restrict__ Bz, T* __restrict__ absB,
+                                                      T* __restrict__ Jx, T* __restrict__ Jy, T* __restrict__ Jz, T* __restrict__ absJ)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    if (i >= nx || j >= ny) return;
+    const long long sy = nx, sz = (long long)nx * ny;
+    const long long q = i + sy * j + sz * k;
+    const T bx = Bx[q], by = By[q], bz = Bz[q];
+    if (absB) absB[q] = sqrt(bx * bx + by * by + bz * bz);
+    T a = T(0), b = T(0), c = T(0);
+    const bool wall = i == 0 || i == nx - 1 || j == 0 || j == ny - 1 || k == nz - 1;
+    if (!wall) {
+        const T dyBz = (Bz[q + sy] - Bz[q - sy]) * i2hy, dxBz = (Bz[q + 1] - Bz[q - 1]) * i2hx;
+        const T dxBy = (By[q + 1] - By[q - 1]) * i2hx, dyBx = (Bx[q + sy] - Bx[q - sy]) * i2hy;
+        T dzBy, dzBx;
+        if (k == 0) {
+            dzBy = (T(-3) * by + T(4) * By[q + sz] - By[q + 2 * sz]) * i2hz;
+            dzBx = (T(-3) * bx + T(4) * Bx[q + sz] - Bx[q + 2 * sz]) * i2hz;
+        } else {
+            dzBy = (By[q + sz] - By[q - sz]) * i2hz;
+            dzBx = (Bx[q + sz] - Bx[q - sz]) * i2hz;
+        }
+        a = (dyBz - dzBy) * imu0; b = (dzBx - dxBz) * imu0; c = (dxBy - dyBx) * imu0;
+    }
+    if (Jx) { Jx[q] = a; Jy[q] = b; Jz[q] = c; }
+    if (absJ) absJ[q] = sqrt(a * a + b * b + c * c);
+}
+
+template <typename T>
+static void diagnostics_t(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ)
+{
+    static bool once = false;
+    if (!once) { prefer_l1(k_diagnostics<T>); once = true; }
+    const long long N = lv.npts();
+    const T* Bp = (const T*)B;
+    T* Jp = (T*)J;
+    const dim3 b(32, 8), g((lv.nx + 31) / 32, (lv.ny + 7) / 8, lv.nz);
+    k_diagnostics<T><<<g, b, 0, c->stream>>>(lv.nx, lv.ny, lv.nz, (T)(1.0 / (2.0 * lv.hx)), (T)(1.0 / (2.0 * lv.hy)), (T)(1.0 / (2.0 * lv.hz)),
+                                             (T)(1.0 / c->opt.mu0), Bp, Bp + N, Bp + 2 * N, (T*)absB, Jp, Jp ? Jp + N : nullptr,
+                                             Jp ? Jp + 2 * N : nullptr, (T*)absJ);
+}
+
+void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ)
+{
+    count_launch(c);
+    if (c->es == 8) diagnostics_t<double>(c, lv, B, absB, J, absJ);
+    else diagnostics_t<float>(c, lv, B, absB, J, absJ);
+}
+
 }  // namespace mhs
