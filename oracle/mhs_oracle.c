@@ -22,7 +22,8 @@
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
  * may build, load or call this file.  It shares no code with the CUDA path.
- * Every function has a pin in tests/test_oracle_pins.py;
+ * Every function has a pin in tests/test_oracle_pins.py, orc_diagnostics in tests/test_diagnostics.py (see DESIGN.md
+ * "Oracle and its pins");
  * values printed by the paper for P, B, p, rho do not exist (PAPER.md has none), so
  * "paper-value parity" is unpinned and closed forms / invariants / brute force replace it.
  *
