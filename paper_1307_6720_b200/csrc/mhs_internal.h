@@ -137,7 +137,7 @@ bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
 void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ);
 
-// ---- tuned 3D kernels (mhs_kernels_fast.cu) and the single-CTA tail (mhs_kernels_tail.cu) ----
+// ---- tuned 3D kernels (mhs_kernels_fast.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);
 bool mid_level(const mhs_ctx* c, const Level& lv);   // small enough to live in the L2: parallelism-bound, gets fine-grained launch shapes
 // mode 0: sweep; 1: sweep + partial sums of the INPUT's ||rhs - L u||^2; 2: partial sums only; 3: the first two sweeps

@@ -634,7 +634,7 @@ static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, cons
     const int planes = co.nz - 2;
     // z-chunks: one wave of resident blocks (the kernel is bound by parallelism before bytes: measured at 257^3, 32 chunks
     // of 4 coarse planes -- 11 fine planes read for 8 -- beat 16 chunks of 8 by 57 -> 41 us); no shorter than 4 coarse planes
-    const int minlen = RC == 2 ? 2 : 4;
+    const int minlen = 4;
     int nzc = (int)std::max<long long>(1, std::min<long long>(planes / minlen > 0 ? planes / minlen : 1, slots / xb));
     const int Kchunk = (planes + nzc - 1) / nzc;
     nzc = (planes + Kchunk - 1) / Kchunk;
@@ -645,17 +645,11 @@ static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, cons
 void launch_resid_restrict_sep(mhs_ctx* c, const Level& f, const void* u, const void* rhs, const Level& co, void* rc, int reverse, const int* done)
 {
     count_launch(c);
-    // mid levels: two coarse rows per thread instead of four -- twice the threads
-    const bool mid = mid_level(c, f);
-#define RS(T)                                                                                        \
-    do {                                                                                             \
-        if (mid) {                                                                                   \
-            if (rhs) resid_restrict_sep_t<T, true, 2>(c, f, u, rhs, co, rc, reverse, done);          \
-            else resid_restrict_sep_t<T, false, 2>(c, f, u, rhs, co, rc, reverse, done);             \
-        } else {                                                                                     \
-            if (rhs) resid_restrict_sep_t<T, true, 4>(c, f, u, rhs, co, rc, reverse, done);          \
-            else resid_restrict_sep_t<T, false, 4>(c, f, u, rhs, co, rc, reverse, done);             \
-        }                                                                                            \
+    // (only big levels come here -- mhs_api.cu restrict_fast; two coarse rows per thread, RC = 2, measured no faster)
+#define RS(T)                                                                                    \
+    do {                                                                                         \
+        if (rhs) resid_restrict_sep_t<T, true, 4>(c, f, u, rhs, co, rc, reverse, done);          \
+        else resid_restrict_sep_t<T, false, 4>(c, f, u, rhs, co, rc, reverse, done);             \
     } while (0)
     if (c->es == 8) RS(double);
     else RS(float);

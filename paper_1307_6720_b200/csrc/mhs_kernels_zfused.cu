@@ -13,12 +13,11 @@
 //   * A CTA owns a tile of ZWY*ZR rows x TC columns and walks up in z.  Stage s of the pipeline lags one plane
 //     behind stage s-1: at step t stage 1 makes sweep-1 values of plane t-1 from the input planes t-2, t-1, t,
 //     stage 2 makes sweep-2 values of plane t-2 from sweep-1 planes t-3, t-2, t-1.  A thread owns a patch of
-//     4 rows x one 128-bit vector and keeps the z-column (below, centre, above) of its patch for every stage in
-//     registers; the step is unrolled three times so that the three register sets rotate by renaming, not by
-//     moves.  In-plane neighbours: rows of its own patch from registers, everything else from shared memory --
+//     8 (fp64) or 4 (fp32) rows x one 128-bit vector and keeps the z-column (below, centre, above) of its patch for
+//     every stage in registers; steps come in pairs whose register sets swap roles by renaming.  In-plane neighbours: rows of its own patch from registers, everything else from shared memory --
 //     the ring slot of the centre plane for stage 1, a double-buffered exchange plane for stage 2 -- with
 //     plain LDS (no shuffles, no lane-dependent branches).  One __syncthreads per plane.
-//   * Every stage shrinks the valid region by one row/plane at tile and chunk edges: a tile makes WY*4-2(S-1)
+//   * Every stage shrinks the valid region by one row/plane at tile and chunk edges: a tile makes 16-2(S-1)
 //     output rows, a z-segment is warmed up over S planes.  Walls are held fixed in every stage; the bottom
 //     (data) and top planes pass through every stage by coefficients (A = 1, B = 0), so no branch is needed.
 //   * fp64 uses the expanded update  u' = (1-w) u + Bx (e+w) + By (n+s) + Bz (up+dn) + W f  with per-plane
@@ -451,7 +450,7 @@ __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* til
 
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
-// caller swaps the names (the step is unrolled twice), so no register is ever moved.
+// caller swaps the names (steps come in pairs).
 template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
