@@ -483,6 +483,21 @@ def test_full_size_per_iterate_parity(B, orc):
         assert abs(info["history"][0] - rk) <= 1e-6 * rk
 
 
+def test_full_size_dependent_launch_is_invisible(B):
+    """The bench workload itself (257^3, 40 cycles, default flags) three times with and once without programmatic
+    dependent launch: bitwise the same potential and fields."""
+    w = inputs.config(2)
+    out = []
+    for flags in (B.MHS_FLAG_NO_PDL, 0, 0, 0):
+        with B.Solver.from_workload(w, flags=flags) as S:
+            S.solve_boundary(dev(w.Bz0, torch.float64))
+            info = S.solve_interior(w.tol, w.max_cycles)
+            Bf, p, rho = S.fields()
+            out.append((info["cycles"], S.get_potential().clone(), rho.clone()))
+    for c, P, rho in out[1:]:
+        assert c == out[0][0] and torch.equal(P, out[0][1]) and torch.equal(rho, out[0][2])
+
+
 def test_large_grid_sampled_properties(B, orc):
     """BASELINE configs[2] (257^3, the bench workload) in the launch configuration bench.py times:
     the oracle cannot run the solve in seconds, so check (i) two V-cycle iterates on a z-slab-free
