@@ -28,6 +28,13 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 METRIC = "V-cycles/s (3D, whole path: boundary solve + interior solve to tol + fields) at 257^3 fp64"
+
+
+def metric_name(w):
+    """BASELINE.json's metric is quoted on configs[2] (257^3 fp64, the default); other --config values say their own size."""
+    if (w.nx, w.ny, w.nz, w.dtype) == (257, 257, 257, "f64"):
+        return METRIC
+    return METRIC.replace("257^3 fp64", "%dx%dx%d %s" % (w.nx, w.ny, w.nz, "fp64" if w.dtype == "f64" else "fp32"))
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback
 
 
@@ -151,7 +158,7 @@ def run_reference(args, w, cfg):
     val = tot_c / tot_t
     sample = "%d V-cycles of the 3D interior solve per step at full size (%dx%dx%d), 2D solve and fields untimed" % (
         per_step, w.nx, w.ny, w.nz)
-    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": "V-cycles/s", "n_gpus": args.gpus,
+    out = {"impl": "reference", "metric": metric_name(w), "value": val, "unit": "V-cycles/s", "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
            "cpu_baseline": {"value": val, "unit": "V-cycles/s", "cores": thr, "kind": "oracle", "sample": sample},
@@ -308,7 +315,7 @@ def main():
             "prolong_fused_pass": ({"launches": l_fused, "avg_us": 1e3 * t_fused / l_fused, "algorithmic_bytes": b_fused,
                                     "gbs": b_fused * l_fused / (t_fused * 1e-3) / 1e9} if fused_all and t_fused > 0 else None)}
 
-    out = {"metric": METRIC, "value": c3_all / (ms * 1e-3), "unit": "V-cycles/s", "n_gpus": world, "steps": args.steps,
+    out = {"metric": metric_name(w), "value": c3_all / (ms * 1e-3), "unit": "V-cycles/s", "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": w.dtype, "data": "synthetic", "config": cfg,
            "cycles_per_step": {"boundary_2d": c2 / args.steps, "interior_3d": c3 / args.steps},
