@@ -36,6 +36,17 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
+    # one builder at a time: the ranks of a torchrun job all come here at once on a fresh box
+    import fcntl
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    with open(os.path.join(HERE, "build", ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not force and not _stale():      # somebody else built it while we waited
+            return LIB
+        return _build_locked(verbose)
+
+
+def _build_locked(verbose: bool) -> str:
     objs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     procs = []
