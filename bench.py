@@ -176,6 +176,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2 = 257^3 fp64)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=12.0, help="CPU work of the oracle sample (default ~12 s)")
     ap.add_argument("--flags", type=int, default=0, help="mhs_options.flags (1 = reference kernels)")
     args = ap.parse_args()
 
@@ -332,7 +333,7 @@ def main():
            "kernel_launches_by_class": by_class}
     S.close()
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        v, dtm, thr, nc = oracle_sample(w, 1, min_seconds=12.0)
+        v, dtm, thr, nc = oracle_sample(w, 1, min_seconds=args.cpu_baseline_seconds)
         out["cpu_baseline"] = {"value": v, "unit": "V-cycles/s", "cores": thr, "kind": "oracle",
                                "sample": "%d V-cycles of the 3D interior solve at %dx%dx%d (%.1f s of CPU work); 2D solve and fields not timed"
                                          % (nc, w.nx, w.ny, w.nz, dtm)}
