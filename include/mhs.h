@@ -22,8 +22,11 @@
  *   Memory    "device" pointers are CUDA device pointers on the current device, "host" pointers
  *             are ordinary host memory (pinned for best speed).  The caller owns every buffer it
  *             passes; the library copies what it keeps (f_profile, p_b, rho_b, dfdz) and owns the
- *             context and its internal hierarchy, all allocated in mhs_create -- the solve calls
- *             allocate nothing on the device.
+ *             context and its internal hierarchy, all allocated in mhs_create -- the device-pointer
+ *             calls (mhs_solve_*, mhs_fields, ...) allocate nothing on the device.  The *_host entry
+ *             points are the exception: the first mhs_fields_host* / mhs_get_potential_host call
+ *             allocates a device staging buffer (5N resp. N elements, kept until mhs_destroy), and
+ *             event timing (mhs_options.profile > 0) creates CUDA events on demand and recycles them.
  *   Streams   all work is enqueued on mhs_options.stream (a cudaStream_t; NULL = default stream).
  *             mhs_solve_* return after the last residual norm has been read back (they report
  *             `cycles`); the other calls are asynchronous with respect to the host unless they
@@ -34,7 +37,9 @@
  *             mhs_create fails with MHS_ERR_CUDA.
  *   State     create -> solve_boundary -> solve_interior (repeatable: it CONTINUES from the
  *             current P, so max_cycles = 1 called k times yields iterate k) -> fields.
- *             solve_boundary resets the interior to 0.
+ *             solve_boundary resets the interior to 0.  mhs_solve_interior and
+ *             mhs_fields* before a successful mhs_solve_boundary (MHS_OK or MHS_ERR_NOT_CONVERGED)
+ *             or mhs_set_potential return MHS_ERR_STATE.
  */
 #ifndef MHS_H_
 #define MHS_H_
@@ -123,6 +128,8 @@ typedef struct {
     long long sweeps_l0;              /* Jacobi sweeps applied to the finest 3D level                */
     long long fused_prolong_l0;       /* launches of class MHS_KC_PROLONG_L0 that were prolongation-fused
                                          smoothing passes (prolongation + the first post-sweeps in one pass) */
+    long long xtiled_zsweep;          /* launches of the temporally blocked smoother (any level) whose tiles were
+                                         narrower than a grid row (rows wider than 256 fp64 / 512 fp32 columns)  */
 } mhs_profile;
 
 /* Fill *o with the defaults: fp64, omega 2/3, V(2,2), full coarsening, boundary_tol 1e-10,

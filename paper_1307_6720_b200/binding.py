@@ -62,7 +62,7 @@ class mhs_solve_info(C.Structure):
 
 class mhs_profile(C.Structure):
     _fields_ = [("launches", C.c_longlong * MHS_KC_COUNT), ("ms", C.c_double * MHS_KC_COUNT),
-                ("sweeps_l0", C.c_longlong), ("fused_prolong_l0", C.c_longlong)]
+                ("sweeps_l0", C.c_longlong), ("fused_prolong_l0", C.c_longlong), ("xtiled_zsweep", C.c_longlong)]
 
 
 class MHSError(RuntimeError):
@@ -244,7 +244,7 @@ def mhs_get_profile(h):
     names = [lib().mhs_kernel_class_name(k).decode() for k in range(MHS_KC_COUNT)]
     return dict(launches={n: int(p.launches[k]) for k, n in enumerate(names)},
                 ms={n: float(p.ms[k]) for k, n in enumerate(names)}, sweeps_l0=int(p.sweeps_l0),
-                fused_prolong_l0=int(p.fused_prolong_l0),
+                fused_prolong_l0=int(p.fused_prolong_l0), xtiled_zsweep=int(p.xtiled_zsweep),
                 total_launches=int(sum(p.launches)))
 
 
@@ -274,7 +274,8 @@ class Solver:
     def close(self):
         h, self.h = getattr(self, "h", None), None
         if h and _lib is not None:      # (at interpreter exit the module may already be torn down)
-            _lib.mhs_destroy(h)
+            _lib.mhs_destroy(h)         # (synchronises the copy stream before anything is freed)
+        self._inflight = []
 
     __del__ = close
 
@@ -293,6 +294,7 @@ class Solver:
 
     def host_sync(self):
         mhs_host_sync(self.h)
+        self._inflight = []
 
     def fields(self, B=None, p=None, rho=None, want=("B", "p", "rho"), host=False, wait=True):
         dev = "cpu" if host else "cuda"
@@ -304,6 +306,9 @@ class Solver:
         if rho is None and "rho" in want:
             rho = mk(self.N)
         mhs_fields(self.h, B, p, rho, self.dtype, self.N, host=host, wait=wait)
+        if host and not wait:
+            # the copies are still in flight: the pinned buffers must outlive them even if the caller drops the result
+            self._inflight = getattr(self, "_inflight", []) + [B, p, rho]
         shp = (self.nz, self.ny, self.nx)
         return (None if B is None else B.view(3, *shp), None if p is None else p.view(shp),
                 None if rho is None else rho.view(shp))

@@ -18,6 +18,7 @@ LIB = os.path.join(HERE, "libmhs_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+FLAGS += os.environ.get("MHS_NVCC_FLAGS", "").split()     # (A/B builds of tuning macros, e.g. -DMHS_ZR64=4)
 
 
 def sources():

@@ -389,7 +389,11 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
     }
     if (fuse_norm && l == 0) {
         const int first = zs ? std::min(2, n_pre) : 1;
-        const long long np = smooth(ctx, Ls, l, first, nullptr, true);  // must run even when `done` is about to be raised
+        // Launched behind `done` like every other kernel of the cycle: in the unit that finds the stop rule met the flag is
+        // still down when this pass starts (the flag is raised by the norm_final that follows it), so it runs and leaves the
+        // norm; in the speculative units issued after that one it is skipped.  (Launched unconditionally it would, in those
+        // later units and for an odd number of ping-pong passes per cycle, write into the buffer that holds the final iterate.)
+        const long long np = smooth(ctx, Ls, l, first, done, true);
         norm_final(ctx, lv, l, np, 1);
         smooth(ctx, Ls, l, n_pre - first, done);
     } else {
@@ -451,8 +455,8 @@ mhs_status finish_cycles(mhs_ctx* ctx, double tol, mhs_solve_info* info)
 // Solve loop shared by the 2D and 3D drivers.  Unit q = [norm of iterate q-1 -> stop rule] + [V-cycle q];
 // units run speculatively in chunks behind the device-side stop flag and the host reads the control block
 // once per chunk.  The stop rule (C10) is exact: once the flag is up every later kernel returns at once, and
-// the only kernel that may already have run -- the first pre-sweep, which carries the norm -- writes the
-// ping-pong buffer, never the iterate.  iter_buf[q] remembers which buffer holds iterate q.
+// the only kernel that has already run in the stopping unit -- the first pre-sweep, which carries the norm --
+// writes the ping-pong buffer, never the iterate.  iter_buf[q] remembers which buffer holds iterate q.
 mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_cycles, double r0_known,
                       mhs_solve_info* info)
 {
@@ -665,6 +669,8 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         CK(cudaGetDevice(&dev));
         CK(cudaGetDeviceProperties(&pr, dev));
         ctx->num_sms = pr.multiProcessorCount;
+        ctx->device = dev;
+        ctx->debug = getenv("MHS_DEBUG") != nullptr;
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
     ctx->tail3 = (ref || only2d) ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
@@ -758,6 +764,7 @@ mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solv
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
     if (!(tol >= 0.0)) return fail(ctx, MHS_ERR_INVALID_ARG, "tol must be >= 0");
+    if (!ctx->have_boundary) return fail(ctx, MHS_ERR_STATE, "mhs_solve_interior before a successful mhs_solve_boundary / mhs_set_potential");
     mhs_solve_info local;
     if (!info) info = &local;
     mhs_status st = run_cycles(ctx, ctx->L3, tol, max_cycles, ctx->have_r0 ? ctx->r0_interior : 0.0, info);
@@ -813,6 +820,7 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    if (!ctx->have_boundary) return fail(ctx, MHS_ERR_STATE, "mhs_fields before a successful mhs_solve_boundary / mhs_set_potential");
     if (!B && !p && !rho) return MHS_OK;
     Scope sc(ctx, MHS_KC_FIELDS);
     const Level& l0 = ctx->L3[0];
@@ -843,6 +851,7 @@ mhs_status mhs_fields_host_async(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
     if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
+    if (!ctx->have_boundary) return fail(ctx, MHS_ERR_STATE, "mhs_fields_host before a successful mhs_solve_boundary / mhs_set_potential");
     const size_t nb = (size_t)ctx->L3[0].npts() * ctx->es;
     mhs_status st = ensure_stage(ctx, 5 * nb);
     if (st) return st;
@@ -946,6 +955,7 @@ mhs_status mhs_level_set(mhs_ctx* ctx, int dim, int level, int which, const void
     if (bottom) {
         CK(cudaMemcpyAsync(lv.tmp, lv.u, (size_t)lv.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
         ctx->have_r0 = false;
+        ctx->have_boundary = true;   // (the same as mhs_set_potential)
     }
     CK(cudaGetLastError());
     return MHS_OK;

@@ -11,6 +11,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -82,6 +83,8 @@ struct mhs_ctx {
     mhs_profile prof{};
     int cur_kc = MHS_KC_PACK;  // kernel class the launchers charge
     int num_sms = 148;
+    int device = 0;            // the CUDA device the context was created on
+    bool debug = false;        // MHS_DEBUG was set at create: launch shapes go to stderr
     int tail3 = 1 << 30, tail2 = 1 << 30;  // first level kept in shared memory by the cluster kernel's CTA 0
     int clus3 = 1 << 30, clus2 = 1 << 30;  // first level handled by the cluster kernel (<= tail; mhs_kernels_cluster.cu)
     int cluster_max = 8;                   // largest thread-block cluster the device co-schedules (<= 16)
@@ -94,6 +97,26 @@ struct mhs_ctx {
 namespace mhs {
 
 inline void count_launch(mhs_ctx* c) { c->prof.launches[c->cur_kc] += 1; }
+
+// One-time per-kernel setup (cudaFuncSetAttribute applies to the CURRENT device only) and cached occupancy figures are
+// kept per device: a second context on another GPU of the same process must get its own.  `fn` returns a non-zero int
+// (the cached value); concurrent first calls may both run it -- it is idempotent.
+constexpr int MAX_DEVICES = 64;
+struct PerDevice {
+    std::atomic<int> v[MAX_DEVICES];
+    PerDevice() { for (auto& a : v) a.store(0, std::memory_order_relaxed); }
+};
+template <typename F>
+inline int per_device(PerDevice& pd, const mhs_ctx* c, F fn)
+{
+    const int d = c->device >= 0 && c->device < MAX_DEVICES ? c->device : 0;
+    int x = pd.v[d].load(std::memory_order_acquire);
+    if (!x) {
+        x = fn();
+        pd.v[d].store(x, std::memory_order_release);
+    }
+    return x;
+}
 
 // Kernels that live on the L1 (no dynamic shared memory) say so ONCE: with no stated preference a kernel launched after one
 // that had the SM configured for 220 KB of shared memory (k_zsweep, the cluster kernel's tail) inherits that split and runs

@@ -583,11 +583,8 @@ static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, 
     const size_t smem = (size_t)off * sizeof(T);
 
     auto kern = k_cluster<T, D3>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        set_cluster_attrs(kern);
-        attr_set = true;
-    }
+    static PerDevice attr_set;
+    per_device(attr_set, c, [&] { set_cluster_attrs(kern); return 1; });
     int ncta = 1;
     if (P.nglob > 0) {
         // enough CTAs that a phase of the largest cluster level is a handful of row segments per warp
@@ -608,7 +605,7 @@ static cudaError_t cluster_launch_t(mhs_ctx* c, std::vector<Level>& Ls, int lc, 
     at[1].val.programmaticStreamSerializationAllowed = (c->opt.flags & MHS_FLAG_NO_PDL) ? 0 : 1;
     cfg.attrs = at; cfg.numAttrs = 2;
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, P, done);
-    if (e != cudaSuccess || getenv("MHS_DEBUG"))
+    if (e != cudaSuccess || c->debug)
         fprintf(stderr, "[mhs] k_cluster<%s,%dD> mode %d levels [%d,%d) tail [%d,%d) cluster %d smem %zu: %s\n", sizeof(T) == 8 ? "f64" : "f32",
                 D3 ? 3 : 2, mode, lc, lt, lt, n, ncta, smem, cudaGetErrorString(e));
     return e;

@@ -356,13 +356,13 @@ static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const vo
 {
     constexpr int V = VN<T>::N;
     auto kern = k_smooth_z<T, R, HAS_RHS, STORE, NORM, ZERO2>;
-    static int slots = 0;
-    if (!slots) {
+    static PerDevice slots_pd;
+    const int slots = per_device(slots_pd, c, [&] {
         prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
-        slots = std::max(1, nb) * c->num_sms;
-    }
+        return std::max(1, nb) * c->num_sms;
+    });
     const long long items = (long long)((lv.sy + R - 1) / R) * (lv.sx / V);
     const long long xb = (items + 127) / 128;
     const int planes = lv.nz - 2;
@@ -411,8 +411,8 @@ long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
 
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done)
 {
-    static bool once = false;
-    if (!once) { prefer_l1(k_scale_rhs<double>); prefer_l1(k_scale_rhs<float>); once = true; }
+    static PerDevice once;
+    per_device(once, c, [&] { prefer_l1(k_scale_rhs<double>); prefer_l1(k_scale_rhs<float>); return 1; });
     count_launch(c);
     const int V = c->es == 8 ? 2 : 4;
     dim3 grid((unsigned)((lv.sp / V + 255) / 256), (unsigned)(lv.nz - 2));
@@ -425,13 +425,13 @@ static void resid_restrict_t(mhs_ctx* c, const Level& f, const void* u, const vo
 {
     constexpr int V = VN<T>::N;
     auto kern = k_resid_restrict_z<T, R, HAS_RHS>;
-    static int slots = 0;
-    if (!slots) {
+    static PerDevice slots_pd;
+    const int slots = per_device(slots_pd, c, [&] {
         prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
-        slots = std::max(1, nb) * c->num_sms;
-    }
+        return std::max(1, nb) * c->num_sms;
+    });
     const long long items = (long long)((f.sy + R - 1) / R) * (f.sx / V);
     const long long warps = (items + 1 + 30) / 31;   // lanes 1..31 of each warp carry items
     const long long xb = (warps + 3) / 4;
@@ -464,8 +464,8 @@ void launch_resid_restrict_z(mhs_ctx* c, const Level& f, const void* u, const vo
 
 void launch_prolong_v(mhs_ctx* c, const Level& f, void* u, const Level& co, const void* ec, int reverse, const int* done)
 {
-    static bool once = false;
-    if (!once) { prefer_l1(k_prolong_v<double>); prefer_l1(k_prolong_v<float>); once = true; }
+    static PerDevice once;
+    per_device(once, c, [&] { prefer_l1(k_prolong_v<double>); prefer_l1(k_prolong_v<float>); return 1; });
     count_launch(c);
     const int V = c->es == 8 ? 2 : 4;
     dim3 grid((unsigned)((f.sp / V + 255) / 256), (unsigned)(f.nz - 2));
@@ -624,13 +624,13 @@ static void resid_restrict_sep_t(mhs_ctx* c, const Level& f, const void* u, cons
 {
     constexpr int V = VN<T>::N;
     auto kern = k_resid_restrict_sep<T, RC, HAS_RHS>;
-    static int slots = 0;
-    if (!slots) {
+    static PerDevice slots_pd;
+    const int slots = per_device(slots_pd, c, [&] {
         prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 128, 0);
-        slots = std::max(1, nb) * c->num_sms;
-    }
+        return std::max(1, nb) * c->num_sms;
+    });
     const long long items = (long long)(f.sx / V) * ((co.sy - 1 + RC - 1) / RC);
     const long long xb = (items + 127) / 128;
     const int planes = co.nz - 2;

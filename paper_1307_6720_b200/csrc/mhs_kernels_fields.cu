@@ -227,13 +227,13 @@ static void fields_z_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void
     q.i2mu0 = (T)(1.0 / (2.0 * c->opt.mu0)); q.imu0 = (T)(1.0 / c->opt.mu0); q.ig = (T)(1.0 / c->opt.g);
     q.ft = (const T*)c->prof_tab;
     auto kern = k_fields_z<T>;
-    static int slots = 0;
-    if (!slots) {
+    static PerDevice slots_pd;
+    const int slots = per_device(slots_pd, c, [&] {
         prefer_l1(kern);
         int nb = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 256, 0);
-        slots = std::max(1, nb) * c->num_sms;
-    }
+        return std::max(1, nb) * c->num_sms;
+    });
     const int bx = lv.sx / (32 * V), by = lv.sy / 8;
     const int planes = lv.nz - 2;
     // z-chunks: about two waves of blocks, chunks no shorter than 8 planes (2 warm-up planes each)
@@ -295,8 +295,8 @@ __global__ void __launch_bounds__(256) k_diagnostics(int nx, int ny, int nz, T i
 template <typename T>
 static void diagnostics_t(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ)
 {
-    static bool once = false;
-    if (!once) { prefer_l1(k_diagnostics<T>); once = true; }
+    static PerDevice once;
+    per_device(once, c, [&] { prefer_l1(k_diagnostics<T>); return 1; });
     const long long N = lv.npts();
     const T* Bp = (const T*)B;
     T* Jp = (T*)J;

@@ -330,8 +330,8 @@ long long resnorm_partial_capacity(const Level& lv)
 void launch_norm_final(mhs_ctx* c, long long n, int mode)
 {
     count_launch(c);
-    static bool once = false;
-    if (!once) { prefer_l1(k_norm_final); once = true; }
+    static PerDevice once;
+    per_device(once, c, [&] { prefer_l1(k_norm_final); return 1; });
     launch_pdl(c, k_norm_final, dim3(1), dim3(1024), 0, (const double*)c->partial, n, c->ctl, mode);
 }
 

@@ -38,7 +38,10 @@ template <typename T> struct ZV;
 // along y (a tile has WY*R = 16 patch rows).  fp64: 8 rows x 256 threads x <= 255 registers ("few fat threads": measured
 // 62.5 us per 2-sweep pass at 257^3 against 68 us for 4 rows x 512 threads); fp32, with half the registers per value and the
 // longer difference-form update, is faster the other way round (1025^2 x 257: 632 us against 900 us per pass).
-template <> struct ZV<double> { static constexpr int N = 2, NCO = 6, R = 8, WY = 2; };
+#ifndef MHS_ZR64
+#define MHS_ZR64 8
+#endif
+template <> struct ZV<double> { static constexpr int N = 2, NCO = 6, R = MHS_ZR64, WY = 16 / MHS_ZR64; };
 template <> struct ZV<float> { static constexpr int N = 4, NCO = 4, R = 4, WY = 4; };
 
 // Tile geometry is a compile-time function of WXT (warps along x), so that every shared-memory stride is an immediate:
@@ -257,6 +260,8 @@ struct ZCtx {
     int zoff;                     // ring position of input plane k is zoff + k
     int omask;                    // rows of the patch that are stored (output rows, output columns)
     bool cw0;                     // element 0 of the patch is a wall column
+    bool swp;                     // this lane fetches its x-neighbours in swapped order (see z_step)
+    uint32_t eo1, eo2;            // byte offsets, from a row's vector, of the first / second x-neighbour load
     double acc;
     // prolongation-fused variant
     uint32_t in_base, ce_base;    // shared-space addresses of ring slot 0 / coarse ring slot 0
@@ -486,19 +491,26 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
         ZVec<T> up0, edge1, edge2, f1, f2;
         T w, e, w2, e2;
     };
+    // x-neighbours (the element left of the vector, w, and the one right of it, e) are single elements 16 bytes apart
+    // from lane to lane: a warp-wide load of all the w (or all the e) touches only every other 8-byte bank pair (fp64; one
+    // bank in four in fp32) and takes twice the wavefronts it needs -- measured, these loads were 40 % of the kernel's
+    // shared-memory wavefronts, and the shared-memory pipe is its busiest unit.  So lanes 8-15 and 24-31 fetch e where the
+    // others fetch w and the other way round in the second load: every half-warp then covers all banks.  The two values are
+    // put back in order with selects (z.swp).
+    const uint32_t a_cen1 = a_cen + z.eo1, a_cen2 = a_cen + z.eo2, a_exr1 = a_exr + z.eo1, a_exr2 = a_exr + z.eo2;
     auto load_row = [&](int r, RowIn& q) {
         const long long grow = (long long)r * p.sx;
         if (!ZERO) {
             q.up0 = lds_vec<T>(a_new + r * rowb);
-            q.w = lds_one<T>(a_cen + r * rowb - ES);
-            q.e = lds_one<T>(a_cen + r * rowb + V * ES);
+            q.w = lds_one<T>(a_cen1 + r * rowb);
+            q.e = lds_one<T>(a_cen2 + r * rowb);
             if (r == ZR - 1) q.edge1 = lds_vec<T>(a_cen + ZR * rowb);
             if (r == 0) q.edge1 = lds_vec<T>(a_cen - rowb);
         }
         if (HAS_RHS) q.f1 = zld(z.f1 + grow);
         if (S == 2) {
-            q.w2 = lds_one<T>(a_exr + r * rowb - ES);
-            q.e2 = lds_one<T>(a_exr + r * rowb + V * ES);
+            q.w2 = lds_one<T>(a_exr1 + r * rowb);
+            q.e2 = lds_one<T>(a_exr2 + r * rowb);
             if (r == ZR - 1) q.edge2 = lds_vec<T>(a_exr + ZR * rowb);
             if (r == 0) q.edge2 = lds_vec<T>(a_exr - rowb);
             if (HAS_RHS) q.f2 = zld(z.f1 - p.sp + grow);
@@ -521,7 +533,8 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             const ZVec<T> nn = r == ZR - 1 ? in.edge1 : c0.r[r + 1 < ZR ? r + 1 : r];
             const ZVec<T> ss = r == 0 ? in.edge1 : c0.r[r > 0 ? r - 1 : 0];
             float rs = 0.f;
-            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], in.w, in.e, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
+            const T w1 = z.swp ? in.e : in.w, e1 = z.swp ? in.w : in.e;
+            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], w1, e1, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
             if (z.cw0) o1.v[0] = c0.r[r].v[0];
             if (NORM && (m1 & (1 << r))) {
                 if (sizeof(T) == 8) {
@@ -545,7 +558,8 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             const ZVec<T> nn = r == ZR - 1 ? in.edge2 : c1.r[r + 1 < ZR ? r + 1 : r];
             const ZVec<T> ss = r == 0 ? in.edge2 : c1.r[r > 0 ? r - 1 : 0];
             float rs;
-            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], in.w2, in.e2, nn, ss, o1, dn1.r[r], in.f2, o2, false, rs);
+            const T w2 = z.swp ? in.e2 : in.w2, e2 = z.swp ? in.w2 : in.e2;
+            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], w2, e2, nn, ss, o1, dn1.r[r], in.f2, o2, false, rs);
             if (z.cw0) o2.v[0] = c1.r[r].v[0];
             if (m2 & (1 << r)) zst(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
@@ -604,6 +618,9 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     z.in_own = smem_u32(IN + (wy * ZR + 1) * TC + cx0);
     z.ex_own = smem_u32(EX + (wy * ZR + 1) * TC + cx0);
     z.acc = 0.0;
+    z.swp = (lane & 8) != 0;
+    z.eo1 = z.swp ? (uint32_t)(V * sizeof(T)) : (uint32_t)(0u - (uint32_t)sizeof(T));
+    z.eo2 = z.swp ? (uint32_t)(0u - (uint32_t)sizeof(T)) : (uint32_t)(V * sizeof(T));
     z.in_base = smem_u32(IN);
     z.ce_base = PRO ? smem_u32(CE) : 0u;
     z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0;
@@ -783,14 +800,14 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
                            const void* ec = nullptr, long long csp = 0)
 {
     auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>;
-    static bool attr = false;
-    if (!attr) {
+    static PerDevice attr;
+    per_device(attr, c, [&] {
         cudaFuncAttributes fa;
         size_t stat = 4096;
         if (cudaFuncGetAttributes(&fa, kern) == cudaSuccess) stat = fa.sharedSizeBytes;
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(227 * 1024 - stat));
-        attr = true;
-    }
+        return 1;
+    });
     ZP<T> p;
     p.sx = lv.sx; p.sy = lv.sy; p.nz = lv.nz; p.sp = lv.sp;
     p.tab = (const T*)lv.tab;
@@ -804,8 +821,9 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
     p.ec = (const T*)ec; p.csp = csp;
+    if (z.ntx > 1) c->prof.xtiled_zsweep += 1;
     launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZV<T>::WY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
-    if (getenv("MHS_DEBUG")) {
+    if (c->debug) {
         cudaError_t e = cudaPeekAtLastError();
         fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
                 sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, (int)PRO, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
