@@ -91,6 +91,8 @@ def lib():
         L.orc_fields.argtypes = g3 + [_d, _p, _p, _p, _p, _d, _d, _p, _p, _p, _p, _p, _p]
         L.orc_diagnostics.argtypes = g3 + [_d, _p, _p, _p, _p, _p, _p, _p, _p]
         L.orc_diagnostics.restype = None
+        L.orc_fieldlines.argtypes = g3 + [_p, _p, _p, _i, _p, _d, _i, _i, _d, _p, C.POINTER(C.c_int)]
+        L.orc_fieldlines.restype = None
         _lib = L
     return _lib
 
@@ -315,3 +317,17 @@ def diagnostics(Bx, By, Bz, Lxyz, mu0=0.5):
     out = [np.empty_like(Bx) for _ in range(5)]
     lib().orc_diagnostics(nx, ny, nz, *Lxyz, mu0, _ptr(Bx), _ptr(By), _ptr(Bz), *[_ptr(o) for o in out])
     return tuple(out)
+
+
+def fieldlines(Bx, By, Bz, Lxyz, seeds, step, max_points, direction=1, bmin=0.0):
+    """RK4 field-line integration through the trilinearly interpolated nodal B (Figs 1, 4, 5).
+    seeds: (n, 3) positions (x, y, z) in [0,Lx]x[0,Ly]x[0,Lz].  Returns (lines (n, max_points, 3), npoints (n,))."""
+    Bx, By, Bz = _a(Bx), _a(By), _a(Bz)
+    nz, ny, nx = Bx.shape
+    seeds = _a(seeds).reshape(-1, 3)
+    n = seeds.shape[0]
+    lines = np.full((n, max_points, 3), np.nan)
+    npts = np.zeros(n, dtype=np.int32)
+    lib().orc_fieldlines(nx, ny, nz, *Lxyz, _ptr(Bx), _ptr(By), _ptr(Bz), n, _ptr(seeds), float(step), int(max_points),
+                         int(direction), float(bmin), _ptr(lines), npts.ctypes.data_as(C.POINTER(C.c_int)))
+    return lines, npts

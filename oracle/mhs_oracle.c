@@ -657,3 +657,87 @@ void orc_diagnostics(int nx, int ny, int nz, double Lx, double Ly, double Lz, do
                 absJ[q] = sqrt(a * a + b * b + c * c);
             }
 }
+
+/* ------------------------------------------------------------------------------------
+ * Field-line integration (SURVEY 8(f) NEXT-4; the field lines of the paper's Figs 1, 4, 5, PAPER.md:142-144, :158-186;
+ * the paper draws them with IDL, and names no integrator -- reading C24 in DESIGN.md):
+ *     dx/ds = dir * B(x) / |B(x)|          (s = arc length, dir = +1 / -1)
+ * B(x) between the nodes = trilinear interpolation of the nodal B that orc_fields returns; classical fourth-order
+ * Runge-Kutta with a fixed arc-length step `step`.  Point 0 is the seed; a line ends when a Runge-Kutta stage or the new
+ * point falls outside the box [0,Lx]x[0,Ly]x[0,Lz], when |B| <= bmin at a stage (a null), or at max_points.
+ * A seed outside the box gives 0 points.  lines: nseeds x max_points x 3 (x, y, z), points beyond npoints[s] untouched.
+ * Every product-sum is written with fma() in the order the formulas below show, so that an implementation that does the
+ * same gets the same points bit for bit (the exit tests decide an integer).
+ * ---------------------------------------------------------------------------------- */
+static int fl_inside(double x, double y, double z, double Lx, double Ly, double Lz)
+{
+    return x >= 0.0 && x <= Lx && y >= 0.0 && y <= Ly && z >= 0.0 && z <= Lz;
+}
+
+/* trilinear sample of one component a at (x,y,z): cell (i,j,k) = floor(x/hx) clamped to [0, n-2], weights t = x/hx - i;
+ * lerp along x, then y, then z, each as fma(t, b - a, a) */
+static double fl_sample(const double *a, int nx, int ny, int nz, double ihx, double ihy, double ihz,
+                        double x, double y, double z)
+{
+    double fx = x * ihx, fy = y * ihy, fz = z * ihz;
+    int i = (int)floor(fx), j = (int)floor(fy), k = (int)floor(fz);
+    if (i < 0) i = 0; if (i > nx - 2) i = nx - 2;
+    if (j < 0) j = 0; if (j > ny - 2) j = ny - 2;
+    if (k < 0) k = 0; if (k > nz - 2) k = nz - 2;
+    double tx = fx - i, ty = fy - j, tz = fz - k;
+    double a000 = a[I3(i, j, k)], a100 = a[I3(i + 1, j, k)], a010 = a[I3(i, j + 1, k)], a110 = a[I3(i + 1, j + 1, k)];
+    double a001 = a[I3(i, j, k + 1)], a101 = a[I3(i + 1, j, k + 1)], a011 = a[I3(i, j + 1, k + 1)], a111 = a[I3(i + 1, j + 1, k + 1)];
+    double b00 = fma(tx, a100 - a000, a000), b10 = fma(tx, a110 - a010, a010);
+    double b01 = fma(tx, a101 - a001, a001), b11 = fma(tx, a111 - a011, a011);
+    double c0 = fma(ty, b10 - b00, b00), c1 = fma(ty, b11 - b01, b01);
+    return fma(tz, c1 - c0, c0);
+}
+
+/* unit tangent dir*B/|B| at (x,y,z); returns 0 if outside the box or |B| <= bmin */
+static int fl_tangent(const double *Bx, const double *By, const double *Bz, int nx, int ny, int nz, double Lx, double Ly,
+                      double Lz, double ihx, double ihy, double ihz, double dir, double bmin, double x, double y, double z,
+                      double *t)
+{
+    if (!fl_inside(x, y, z, Lx, Ly, Lz)) return 0;
+    double bx = fl_sample(Bx, nx, ny, nz, ihx, ihy, ihz, x, y, z);
+    double by = fl_sample(By, nx, ny, nz, ihx, ihy, ihz, x, y, z);
+    double bz = fl_sample(Bz, nx, ny, nz, ihx, ihy, ihz, x, y, z);
+    double m = sqrt(fma(bz, bz, fma(by, by, bx * bx)));
+    if (!(m > bmin)) return 0;
+    double s = dir / m;
+    t[0] = bx * s; t[1] = by * s; t[2] = bz * s;
+    return 1;
+}
+
+void orc_fieldlines(int nx, int ny, int nz, double Lx, double Ly, double Lz, const double *Bx, const double *By,
+                    const double *Bz, int nseeds, const double *seeds, double step, int max_points, int direction,
+                    double bmin, double *lines, int *npoints)
+{
+    double ihx = (nx - 1) / Lx, ihy = (ny - 1) / Ly, ihz = (nz - 1) / Lz;
+    double dir = direction < 0 ? -1.0 : 1.0, h = step, h2 = 0.5 * step, h6 = step / 6.0;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int s = 0; s < nseeds; ++s) {
+        double x = seeds[3 * s], y = seeds[3 * s + 1], z = seeds[3 * s + 2];
+        double *out = lines + (size_t)s * max_points * 3;
+        int n = 0;
+        if (max_points > 0 && fl_inside(x, y, z, Lx, Ly, Lz)) {
+            out[0] = x; out[1] = y; out[2] = z;
+            n = 1;
+            while (n < max_points) {
+                double k1[3], k2[3], k3[3], k4[3];
+                if (!fl_tangent(Bx, By, Bz, nx, ny, nz, Lx, Ly, Lz, ihx, ihy, ihz, dir, bmin, x, y, z, k1)) break;
+                if (!fl_tangent(Bx, By, Bz, nx, ny, nz, Lx, Ly, Lz, ihx, ihy, ihz, dir, bmin, fma(h2, k1[0], x), fma(h2, k1[1], y), fma(h2, k1[2], z), k2)) break;
+                if (!fl_tangent(Bx, By, Bz, nx, ny, nz, Lx, Ly, Lz, ihx, ihy, ihz, dir, bmin, fma(h2, k2[0], x), fma(h2, k2[1], y), fma(h2, k2[2], z), k3)) break;
+                if (!fl_tangent(Bx, By, Bz, nx, ny, nz, Lx, Ly, Lz, ihx, ihy, ihz, dir, bmin, fma(h, k3[0], x), fma(h, k3[1], y), fma(h, k3[2], z), k4)) break;
+                double xn = fma(h6, (k1[0] + k4[0]) + 2.0 * (k2[0] + k3[0]), x);
+                double yn = fma(h6, (k1[1] + k4[1]) + 2.0 * (k2[1] + k3[1]), y);
+                double zn = fma(h6, (k1[2] + k4[2]) + 2.0 * (k2[2] + k3[2]), z);
+                if (!fl_inside(xn, yn, zn, Lx, Ly, Lz)) break;
+                x = xn; y = yn; z = zn;
+                out[3 * n] = x; out[3 * n + 1] = y; out[3 * n + 2] = z;
+                ++n;
+            }
+        }
+        npoints[s] = n;
+    }
+}
