@@ -169,6 +169,22 @@ mhs_status mhs_fields_host(mhs_ctx *ctx, void *B_host, void *p_host, void *rho_h
  * B_device: the 3*N values mhs_fields wrote (Bx | By | Bz).  absB, absJ: N values; J: 3*N (jx | jy | jz); any of the three
  * outputs may be NULL (skipped).  All device, dense, the context's dtype. */
 mhs_status mhs_diagnostics(mhs_ctx *ctx, const void *B_device, void *absB_device, void *J_device, void *absJ_device);
+/* Field-line integration (the field lines of the paper's Figs 1, 4, 5; reading C24): for every
+ * seed the line  dx/ds = direction * B(x) / |B(x)|  (s = arc length) is followed with the classical fourth-order Runge-Kutta
+ * method and a fixed step `step`; B between the nodes is the trilinear interpolation of the nodal B (cell = floor(x/hx) clamped
+ * to the grid, lerp along x, then y, then z).  Point 0 of a line is its seed; the line ends when a Runge-Kutta stage or the new
+ * point lies outside [0,Lx]x[0,Ly]x[0,Lz], when |B| <= bmin at a stage (a null point), or at max_points points.
+ * A seed outside the box gives 0 points.  Nothing is rendered: the polylines are left in a device buffer.
+ *   B_device     3*N values as mhs_fields wrote them (Bx | By | Bz), dense, the context's dtype
+ *   seeds_device 3*nseeds values (x, y, z per seed), the context's dtype, coordinates in [0,Lx]x[0,Ly]x[0,Lz]
+ *   lines_device nseeds * max_points * 3 values: point n of line s at [(s*max_points + n)*3 + {0,1,2}]; entries beyond a
+ *                line's point count are left untouched
+ *   npoints_device nseeds ints: points written per line
+ * direction: +1 along B, -1 against it.  step > 0, max_points >= 1, bmin >= 0.  Asynchronous on the context's stream.
+ * In fp64 every product-sum is one fma, in the order: lerps fma(t, b - a, a); |B|^2 = fma(bz,bz, fma(by,by, bx*bx));
+ * stage points fma(step/2 or step, k, x); new point fma(step/6, (k1 + k4) + 2 (k2 + k3), x). */
+mhs_status mhs_fieldlines(mhs_ctx *ctx, const void *B_device, int nseeds, const void *seeds_device, double step, int max_points,
+                          int direction, double bmin, void *lines_device, int *npoints_device);
 /* The same without waiting for the copies: the fields are computed on the context's stream into the library's staging
  * buffer and copied to the (pinned) host buffers on a separate copy stream; the call returns as soon as that is enqueued,
  * so the next mhs_solve_* can run while the results of this one travel over PCIe.  The host buffers must not be read, and

@@ -91,6 +91,14 @@ def lib():
         L.orc_fields.argtypes = g3 + [_d, _p, _p, _p, _p, _d, _d, _p, _p, _p, _p, _p, _p]
         L.orc_diagnostics.argtypes = g3 + [_d, _p, _p, _p, _p, _p, _p, _p, _p]
         L.orc_diagnostics.restype = None
+        L.orc_zline3.argtypes = g3 + [_p, _d, _d, _p, _p, _p]
+        L.orc_zline3.restype = None
+        L.orc_vcycle3s.restype = _i
+        L.orc_vcycle3s.argtypes = g3 + [_p, _d, _d, _i, _i, _i, _i, _i, _p, _p]
+        L.orc_fmg_interior.restype = _i
+        L.orc_fmg_interior.argtypes = g3 + [_p, _d, _d, _i, _i, _i, _i, _i, _p]
+        L.orc_solve_interior_opt.restype = _i
+        L.orc_solve_interior_opt.argtypes = g3 + [_p, _d, _d, _i, _i, _i, _i, _i, _d, _i, _p, _p, _p, _i]
         L.orc_fieldlines.argtypes = g3 + [_p, _p, _p, _i, _p, _d, _i, _i, _d, _p, C.POINTER(C.c_int)]
         L.orc_fieldlines.restype = None
         _lib = L
@@ -331,3 +339,40 @@ def fieldlines(Bx, By, Bz, Lxyz, seeds, step, max_points, direction=1, bmin=0.0)
     lib().orc_fieldlines(nx, ny, nz, *Lxyz, _ptr(Bx), _ptr(By), _ptr(Bz), n, _ptr(seeds), float(step), int(max_points),
                          int(direction), float(bmin), _ptr(lines), npts.ctypes.data_as(C.POINTER(C.c_int)))
     return lines, npts
+
+
+# ---- solver variants: z-line Jacobi smoothing, full-multigrid start -------------------------------
+def zline3(u, rhs, c, alpha, omega, Lxyz):
+    """One weighted z-line Jacobi sweep: unew = u + omega T^-1 (rhs - L u), T = the z-tridiagonal part of L."""
+    u = _a(u); c = _a(c); rhs = None if rhs is None else _a(rhs)
+    un = np.empty_like(u)
+    lib().orc_zline3(*_g3(u, Lxyz), _ptr(c), alpha, omega, _ptr(u), _ptr(rhs), _ptr(un))
+    return un
+
+
+def vcycle3s(u, rhs, c, alpha, Lxyz, omega=2.0 / 3.0, n_pre=2, n_post=2, max_levels=0, level=0, smoother=0):
+    u = _a(u).copy(); c = _a(c); rhs = None if rhs is None else _a(rhs)
+    if lib().orc_vcycle3s(*_g3(u, Lxyz), _ptr(c), alpha, omega, n_pre, n_post, level, max_levels, smoother, _ptr(u), _ptr(rhs)):
+        raise ArithmeticError("coarse solve failed")
+    return u
+
+
+def fmg_interior(P, f, alpha, Lxyz, omega=2.0 / 3.0, n_pre=2, n_post=2, max_levels=0, smoother=0, n_fmg=1):
+    """Full-multigrid initial guess for step 3 from the bottom-plane data in P (the interior of P is ignored)."""
+    P = _a(P).copy(); f = _a(f)
+    nz, ny, nx = P.shape
+    if lib().orc_fmg_interior(nx, ny, nz, *Lxyz, _ptr(f), alpha, omega, n_pre, n_post, max_levels, smoother, n_fmg, _ptr(P)):
+        raise ArithmeticError("coarse solve failed")
+    return P
+
+
+def solve_interior_opt(P, f, alpha, Lxyz, omega=2.0 / 3.0, n_pre=2, n_post=2, max_levels=0, smoother=0, fmg=0,
+                       tol=1e-10, max_cycles=100, r0=0.0):
+    P = _a(P).copy(); f = _a(f)
+    nz, ny, nx = P.shape
+    hist = np.zeros(max(max_cycles, 1)); r0c = C.c_double(r0)
+    n = lib().orc_solve_interior_opt(nx, ny, nz, *Lxyz, _ptr(f), alpha, omega, n_pre, n_post, max_levels, smoother, fmg,
+                                     tol, max_cycles, _ptr(P), C.cast(C.byref(r0c), _p), _ptr(hist), hist.size)
+    if n < 0:
+        raise ArithmeticError("coarse solve failed")
+    return P, dict(cycles=n, r0=r0c.value, history=hist[:n].copy())

@@ -741,3 +741,172 @@ void orc_fieldlines(int nx, int ny, int nz, double Lx, double Ly, double Lz, con
         npoints[s] = n;
     }
 }
+
+/* ====================================================================================
+ *  Solver variants inside "a multigrid method" (SURVEY 8(f) NEXT-3; PAPER.md:90 "multigrid methods", :148-156: the
+ *  paper's xi_2 profile takes 1 - xi down to 0.05 near the base, where the z-coupling of eq (8) dominates the horizontal
+ *  one and point relaxation smooths poorly).  These change the iterates, so they are options with their own pins; the
+ *  functions above are untouched.  Readings C25-C27 in DESIGN.md.
+ * ================================================================================== */
+
+/* One weighted z-LINE Jacobi sweep (reading C25).  Split L = T + O: T couples a node to itself and to its two z-neighbours,
+ *     (T u)_ijk = (u_{k+1} + u_{k-1})/hz^2 + D_k u_k,      D_k the diagonal of L on plane k,
+ * O is the rest (the four horizontal neighbours).  All lines are relaxed simultaneously from the old values (two arrays,
+ * as the paper's Jacobi):   unew = u + omega * d,   T d = rhs - L u  on every line (i,j), d = 0 at k = 0, nz-1.
+ * T is the same tridiagonal matrix for every line; it is solved by the Thomas algorithm (no pivoting: |D_k| > 2/hz^2
+ * whenever the operator is definite).  Boundary nodes: unew = u. */
+void orc_zline3(int nx, int ny, int nz, double hx, double hy, double hz, const double *c,
+                double alpha, double omega, const double *u, const double *rhs, double *unew)
+{
+    size_t N = (size_t)nx * ny * nz;
+    int m = nz - 2;
+    double a = 1.0 / (hz * hz);
+    double *r = (double *)malloc(sizeof(double) * N);
+    orc_residual3(nx, ny, nz, hx, hy, hz, c, alpha, u, rhs, r);
+    memcpy(unew, u, sizeof(double) * N); /* boundary branch */
+#pragma omp parallel for schedule(static)
+    for (int j = 1; j < ny - 1; ++j) {
+        double *cp = (double *)malloc(sizeof(double) * (size_t)(m + 2));
+        double *dp = (double *)malloc(sizeof(double) * (size_t)(m + 2));
+        for (int i = 1; i < nx - 1; ++i) {
+            /* forward elimination, k = 1 .. nz-2 */
+            double den = diag3(hx, hy, hz, c[1], alpha);
+            cp[1] = a / den;
+            dp[1] = r[I3(i, j, 1)] / den;
+            for (int k = 2; k <= m; ++k) {
+                den = diag3(hx, hy, hz, c[k], alpha) - a * cp[k - 1];
+                cp[k] = a / den;
+                dp[k] = (r[I3(i, j, k)] - a * dp[k - 1]) / den;
+            }
+            /* back substitution */
+            double d = dp[m];
+            unew[I3(i, j, m)] = u[I3(i, j, m)] + omega * d;
+            for (int k = m - 1; k >= 1; --k) {
+                d = dp[k] - cp[k] * d;
+                unew[I3(i, j, k)] = u[I3(i, j, k)] + omega * d;
+            }
+        }
+        free(cp); free(dp);
+    }
+    free(r);
+}
+
+/* One smoothing sweep by name: 0 = point Jacobi (orc_jacobi3), 1 = z-line Jacobi (orc_zline3). */
+static void smooth3(int smoother, int nx, int ny, int nz, double hx, double hy, double hz, const double *c, double alpha,
+                    double omega, const double *u, const double *rhs, double *unew)
+{
+    if (smoother == 1) orc_zline3(nx, ny, nz, hx, hy, hz, c, alpha, omega, u, rhs, unew);
+    else orc_jacobi3(nx, ny, nz, hx, hy, hz, c, alpha, omega, u, rhs, unew);
+}
+
+/* orc_vcycle3 with the smoother as an option (the same steps in the same order; smoother = 0 reproduces it). */
+int orc_vcycle3s(int nx, int ny, int nz, double hx, double hy, double hz, const double *c, double alpha, double omega,
+                 int n_pre, int n_post, int level, int max_levels, int smoother, double *u, const double *rhs)
+{
+    if (orc_is_coarsest(nx, ny, nz, level, max_levels))
+        return orc_direct3(nx, ny, nz, hx, hy, hz, c, alpha, u, rhs);
+    size_t N = (size_t)nx * ny * nz;
+    double *tmp = (double *)malloc(sizeof(double) * N);
+    double *r = (double *)malloc(sizeof(double) * N);
+    for (int s = 0; s < n_pre; ++s) {
+        smooth3(smoother, nx, ny, nz, hx, hy, hz, c, alpha, omega, u, rhs, tmp);
+        memcpy(u, tmp, sizeof(double) * N);
+    }
+    orc_residual3(nx, ny, nz, hx, hy, hz, c, alpha, u, rhs, r);
+    int cx = (nx - 1) / 2 + 1, cy = (ny - 1) / 2 + 1, cz = (nz - 1) / 2 + 1;
+    size_t Nc = (size_t)cx * cy * cz;
+    double *rc = (double *)malloc(sizeof(double) * Nc);
+    double *ec = (double *)calloc(Nc, sizeof(double));
+    double *cc = (double *)malloc(sizeof(double) * (size_t)cz);
+    for (int K = 0; K < cz; ++K) cc[K] = c[2 * K];
+    orc_restrict3(nx, ny, nz, r, rc);
+    int st = orc_vcycle3s(cx, cy, cz, 2.0 * hx, 2.0 * hy, 2.0 * hz, cc, alpha, omega, n_pre, n_post, level + 1, max_levels,
+                          smoother, ec, rc);
+    orc_prolong_add3(nx, ny, nz, ec, u);
+    for (int s = 0; s < n_post; ++s) {
+        smooth3(smoother, nx, ny, nz, hx, hy, hz, c, alpha, omega, u, rhs, tmp);
+        memcpy(u, tmp, sizeof(double) * N);
+    }
+    free(tmp); free(r); free(rc); free(ec); free(cc);
+    return st;
+}
+
+/* Full-multigrid start (reading C26): the interior of P (bottom plane = data, as for orc_solve_interior) is replaced by
+ * an initial guess built from the coarse grids upwards instead of zero:
+ *   level l carries the bottom data by injection, P_l(I,J,0) = P(2^l I, 2^l J, 0), zero on sides and top;
+ *   coarsest level: exact solve;   level l < coarsest: u_l = trilinear interpolation of u_{l+1} at the interior nodes
+ *   (its bottom plane is the injected data), followed by n_fmg V-cycles of eq (8) on level l (rhs = 0).
+ * Level 0 included: on return P is the FMG iterate; the caller goes on with ordinary V-cycles.  Returns 0 / -1. */
+int orc_fmg_interior(int nx, int ny, int nz, double Lx, double Ly, double Lz, const double *f, double alpha, double omega,
+                     int n_pre, int n_post, int max_levels, int smoother, int n_fmg, double *P)
+{
+    int lnx[32], lny[32], lnz[32], nl = 0;
+    {
+        int ax = nx, ay = ny, az = nz;
+        for (;;) {
+            lnx[nl] = ax; lny[nl] = ay; lnz[nl] = az;
+            ++nl;
+            if (orc_is_coarsest(ax, ay, az, nl - 1, max_levels)) break;
+            ax = (ax - 1) / 2 + 1; ay = (ay - 1) / 2 + 1; az = (az - 1) / 2 + 1;
+        }
+    }
+    double *cl[32], *ul[32];
+    for (int l = 0; l < nl; ++l) {
+        int s = 1 << l;
+        cl[l] = (double *)malloc(sizeof(double) * (size_t)lnz[l]);
+        for (int K = 0; K < lnz[l]; ++K) cl[l][K] = 1.0 + f[(size_t)s * K];
+        ul[l] = (double *)calloc((size_t)lnx[l] * lny[l] * lnz[l], sizeof(double));
+        for (int J = 0; J < lny[l]; ++J)
+            for (int I = 0; I < lnx[l]; ++I)
+                ul[l][(size_t)I + (size_t)lnx[l] * J] = P[(size_t)(s * I) + (size_t)nx * (size_t)(s * J)];
+    }
+    int st = 0;
+    for (int l = nl - 1; l >= 0 && st == 0; --l) {
+        double s = (double)(1 << l);
+        double hx = s * Lx / (nx - 1), hy = s * Ly / (ny - 1), hz = s * Lz / (nz - 1);
+        if (l == nl - 1) {
+            st = orc_direct3(lnx[l], lny[l], lnz[l], hx, hy, hz, cl[l], alpha, ul[l], NULL);
+        } else {
+            orc_prolong_add3(lnx[l], lny[l], lnz[l], ul[l + 1], ul[l]); /* interior of ul[l] is zero: this IS interpolation */
+            for (int q = 0; q < n_fmg && st == 0; ++q)
+                st = orc_vcycle3s(lnx[l], lny[l], lnz[l], hx, hy, hz, cl[l], alpha, omega, n_pre, n_post, l, max_levels,
+                                  smoother, ul[l], NULL);
+        }
+    }
+    memcpy(P, ul[0], sizeof(double) * (size_t)nx * ny * nz);
+    for (int l = 0; l < nl; ++l) { free(cl[l]); free(ul[l]); }
+    return st;
+}
+
+/* orc_solve_interior with the variants as options: smoother (0 point, 1 z-line Jacobi) and fmg (0: start from the zero
+ * interior as the paper's step 1 says;  n > 0: full-multigrid start with n V-cycles per level).  r0 is ALWAYS
+ * the residual norm of the zero-interior iterate (bottom data only), so tolerances mean the same with and without FMG. */
+int orc_solve_interior_opt(int nx, int ny, int nz, double Lx, double Ly, double Lz, const double *f, double alpha,
+                           double omega, int n_pre, int n_post, int max_levels, int smoother, int fmg, double tol,
+                           int max_cycles, double *P, double *r0_io, double *history, int hist_len)
+{
+    double hx = Lx / (nx - 1), hy = Ly / (ny - 1), hz = Lz / (nz - 1);
+    double *c = (double *)malloc(sizeof(double) * (size_t)nz);
+    for (int k = 0; k < nz; ++k) c[k] = 1.0 + f[k];
+    double r0 = *r0_io;
+    if (!(r0 > 0.0)) {
+        r0 = orc_resnorm3(nx, ny, nz, hx, hy, hz, c, alpha, P, NULL);
+        *r0_io = r0;
+    }
+    int k = 0;
+    if (fmg > 0) {
+        if (orc_fmg_interior(nx, ny, nz, Lx, Ly, Lz, f, alpha, omega, n_pre, n_post, max_levels, smoother, fmg, P)) { free(c); return -1; }
+        /* the FMG iterate may already meet the tolerance: history[-] has no slot for it, so it is reported through a cycle
+         * count of 0 only if it does */
+        if (orc_resnorm3(nx, ny, nz, hx, hy, hz, c, alpha, P, NULL) <= tol * r0) { free(c); return 0; }
+    }
+    while (k < max_cycles) {
+        if (orc_vcycle3s(nx, ny, nz, hx, hy, hz, c, alpha, omega, n_pre, n_post, 0, max_levels, smoother, P, NULL)) { free(c); return -1; }
+        double rk = orc_resnorm3(nx, ny, nz, hx, hy, hz, c, alpha, P, NULL);
+        if (k < hist_len) history[k] = rk;
+        ++k;
+        if (rk <= tol * r0) break;
+    }
+    free(c);
+    return k;
+}

@@ -31,7 +31,7 @@ MHS_KC_COUNT = 8
 
 EXPORTS = [
     "mhs_default_options", "mhs_create", "mhs_destroy", "mhs_solve_boundary", "mhs_solve_boundary_host",
-    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_diagnostics", "mhs_get_potential", "mhs_get_potential_host",
+    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_diagnostics", "mhs_fieldlines", "mhs_get_potential", "mhs_get_potential_host",
     "mhs_set_potential", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
     "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
@@ -99,6 +99,7 @@ def lib():
             getattr(L, n).argtypes = [vp, vp, vp, vp]
         L.mhs_host_sync.argtypes = [vp]
         L.mhs_diagnostics.argtypes = [vp, vp, vp, vp, vp]
+        L.mhs_fieldlines.argtypes = [vp, vp, ip, vp, dp, ip, ip, dp, vp, vp]
         for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential"):
             getattr(L, n).argtypes = [vp, vp]
         L.mhs_last_error.argtypes = [vp]
@@ -323,6 +324,17 @@ class Solver:
                                              _dptr(J, self.dtype, 3 * self.N), _dptr(aJ, self.dtype, self.N)))
         shp = (self.nz, self.ny, self.nx)
         return (None if aB is None else aB.view(shp), None if J is None else J.view(3, *shp), None if aJ is None else aJ.view(shp))
+
+    def fieldlines(self, B, seeds, step, max_points, direction=1, bmin=0.0):
+        """Field lines through `seeds` ((n, 3) device tensor of x, y, z) of the field mhs_fields returned.
+        -> (lines (n, max_points, 3), npoints (n,) int32), device tensors; points beyond npoints[s] are NaN."""
+        n = int(seeds.shape[0])
+        lines = torch.full((n, max_points, 3), float("nan"), dtype=self.dtype, device="cuda")
+        npts = torch.zeros(n, dtype=torch.int32, device="cuda")
+        _check(self.h, lib().mhs_fieldlines(self.h, _dptr(B.reshape(-1), self.dtype, 3 * self.N), n,
+                                            _dptr(seeds.reshape(-1), self.dtype, 3 * n), float(step), int(max_points),
+                                            int(direction), float(bmin), C.c_void_p(lines.data_ptr()), C.c_void_p(npts.data_ptr())))
+        return lines, npts
 
     def get_potential(self, out=None):
         if out is None:

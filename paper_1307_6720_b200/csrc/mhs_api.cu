@@ -847,6 +847,21 @@ mhs_status mhs_diagnostics(mhs_ctx* ctx, const void* B, void* absB, void* J, voi
     return MHS_OK;
 }
 
+mhs_status mhs_fieldlines(mhs_ctx* ctx, const void* B, int nseeds, const void* seeds, double step, int max_points, int direction,
+                          double bmin, void* lines, int* npoints)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
+    if (!B || !seeds || !lines || !npoints) return fail(ctx, MHS_ERR_INVALID_ARG, "NULL argument");
+    if (nseeds < 0 || !(step > 0.0) || max_points < 1 || !(bmin >= 0.0) || (direction != 1 && direction != -1))
+        return fail(ctx, MHS_ERR_INVALID_ARG, "need nseeds >= 0, step > 0, max_points >= 1, bmin >= 0, direction = +1 / -1");
+    if (nseeds == 0) return MHS_OK;
+    Scope sc(ctx, MHS_KC_FIELDS);
+    launch_fieldlines(ctx, ctx->L3[0], B, nseeds, seeds, step, max_points, direction, bmin, lines, npoints);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
 mhs_status mhs_fields_host_async(mhs_ctx* ctx, void* B, void* p, void* rho)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;

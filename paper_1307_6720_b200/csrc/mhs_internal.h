@@ -159,6 +159,9 @@ void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void
 bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
 void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ);
+// ---- field-line integration (mhs_kernels_lines.cu) ----
+void launch_fieldlines(mhs_ctx* c, const Level& lv, const void* B, int nseeds, const void* seeds, double step, int max_points, int direction,
+                       double bmin, void* lines, int* npoints);
 
 // ---- tuned 3D kernels (mhs_kernels_fast.cu) ----
 bool fast_ok(const mhs_ctx* c, const Level& lv);
