@@ -83,6 +83,14 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 
+/* mhs_options.smoother (reading C25) */
+#define MHS_SMOOTH_JACOBI 0 /* weighted point Gauss-Jacobi: the paper's relaxation             */
+#define MHS_SMOOTH_ZLINE  1 /* weighted z-line Jacobi, u' = u + omega T^-1 (rhs - L u), T = diagonal of L + its two
+                               z-neighbours, one tridiagonal solve per (i,j) line: for strong (1 - xi) anisotropy --
+                               the paper's xi_2 profile reaches 1 - xi = 0.05.  3D solve only; the 2D
+                               boundary solve keeps point Jacobi.  Every level runs general one-pass kernels (no
+                               temporal blocking, no shared-memory tail).                                          */
+
 typedef struct {
     int dtype;                 /* MHS_F32 / MHS_F64: element type of ALL device/host field arrays      */
     double omega;              /* Jacobi weight (C4); benchmarks use 2/3                               */
@@ -96,6 +104,17 @@ typedef struct {
     void *stream;              /* cudaStream_t                                                         */
     int profile;               /* 1: time every kernel class with CUDA events on `stream`              */
     int flags;                 /* MHS_FLAG_*                                                           */
+    int smoother;              /* MHS_SMOOTH_JACOBI (default) / MHS_SMOOTH_ZLINE                       */
+    int fmg_cycles;            /* 0 (default): the interior starts from P = 0 as the paper's step 1 says.
+                                  n > 0: FULL-MULTIGRID START (reading C26) -- the first mhs_solve_interior after
+                                  mhs_solve_boundary (not after mhs_set_potential: a potential the caller gives is
+                                  continued from) first replaces the interior by a guess built
+                                  from the coarse grids upwards: level l carries the bottom data by injection, the
+                                  coarsest level is solved exactly, every finer level starts from the trilinear
+                                  interpolation of the level below and gets n V-cycles; the ordinary cycles follow.
+                                  r0 stays the residual norm of the zero-interior iterate, so `tol` means the same;
+                                  info.cycles counts the ordinary finest-level cycles only (0 if the FMG iterate
+                                  already meets the tolerance).                                          */
 } mhs_options;
 
 #define MHS_HISTORY_LEN 256
@@ -133,7 +152,7 @@ typedef struct {
 } mhs_profile;
 
 /* Fill *o with the defaults: fp64, omega 2/3, V(2,2), full coarsening, boundary_tol 1e-10,
- * boundary_max_cycles 100, mu0 = 1/2, g = 1 (C16), no profiles, default stream. */
+ * boundary_max_cycles 100, mu0 = 1/2, g = 1 (C16), no profiles, default stream, point Jacobi, no FMG start. */
 void mhs_default_options(mhs_options *o);
 
 /* Build a context: level hierarchy (C8), per-level coefficient tables c_l[k] = 1 + f(z_k) injected
@@ -158,6 +177,16 @@ mhs_status mhs_solve_boundary_host(mhs_ctx *ctx, const void *Bz0_host, mhs_solve
  * r0 is the residual norm of the iterate found at the first call after mhs_solve_boundary /
  * mhs_set_potential and is remembered across continuing calls. */
 mhs_status mhs_solve_interior(mhs_ctx *ctx, double tol, int max_cycles, mhs_solve_info *info);
+
+/* A batch of nb magnetograms on ONE context -- e.g. a time series of the same region feeding an MHD code (
+ * SURVEY 8(f) NEXT-3): for b = 0 .. nb-1 in order the paper's whole procedure, mhs_solve_boundary(Bz0 + b nx ny) ->
+ * mhs_solve_interior(tol, max_cycles) -> whichever outputs are non-NULL, member b at offset b times the member's size:
+ * P (N values per member), B (3N), p (N), rho (N).  All device, dense, the context's dtype.  infos: host array of nb
+ * mhs_solve_info of the interior solves, or NULL.  Member by member the results are those of the separate calls (each
+ * member starts from P = 0).  Returns MHS_OK; MHS_ERR_NOT_CONVERGED if some member reached max_cycles (every
+ * member is still computed and stored); otherwise the first error, with the members before it complete. */
+mhs_status mhs_solve_batch(mhs_ctx *ctx, int nb, const void *Bz0_device, double tol, int max_cycles, void *P_device,
+                           void *B_device, void *p_device, void *rho_device, mhs_solve_info *infos);
 
 /* Field recovery (C13-C15).  B: 3*N values, Bx | By | Bz one after the other;
  * p, rho: N values each, N = nx*ny*nz.  Any of B, p, rho may be NULL (skipped). */
@@ -200,6 +229,11 @@ mhs_status mhs_host_sync(mhs_ctx *ctx);
 mhs_status mhs_get_potential(mhs_ctx *ctx, void *P_device);
 mhs_status mhs_get_potential_host(mhs_ctx *ctx, void *P_host);
 mhs_status mhs_set_potential(mhs_ctx *ctx, const void *P_device);
+
+/* The result of the last mhs_solve_boundary alone: P(x,y,0), nx*ny values, dense (step 2).  Works on a
+ * boundary-only context (nz = 1) too.  The host variant returns after the copy has completed. */
+mhs_status mhs_get_boundary(mhs_ctx *ctx, void *P0_device);
+mhs_status mhs_get_boundary_host(mhs_ctx *ctx, void *P0_host);
 
 const char *mhs_last_error(const mhs_ctx *ctx); /* never NULL; valid until the next call on ctx */
 const char *mhs_status_string(mhs_status s);

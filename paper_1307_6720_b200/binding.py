@@ -24,6 +24,7 @@ MHS_FLAG_UNFUSED_KERNELS = 4
 MHS_FLAG_BIG_LEVEL_KERNELS = 8
 MHS_FLAG_SEPARATE_PROLONG = 16
 MHS_FLAG_NO_PDL = 32
+MHS_SMOOTH_JACOBI, MHS_SMOOTH_ZLINE = 0, 1
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8
 (MHS_OK, MHS_ERR_INVALID_ARG, MHS_ERR_GRID, MHS_ERR_NOT_ELLIPTIC, MHS_ERR_INDEFINITE, MHS_ERR_STATE,
@@ -31,8 +32,8 @@ MHS_KC_COUNT = 8
 
 EXPORTS = [
     "mhs_default_options", "mhs_create", "mhs_destroy", "mhs_solve_boundary", "mhs_solve_boundary_host",
-    "mhs_solve_interior", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_diagnostics", "mhs_fieldlines", "mhs_get_potential", "mhs_get_potential_host",
-    "mhs_set_potential", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
+    "mhs_solve_interior", "mhs_solve_batch", "mhs_fields", "mhs_fields_host", "mhs_fields_host_async", "mhs_host_sync", "mhs_diagnostics", "mhs_fieldlines", "mhs_get_potential", "mhs_get_potential_host",
+    "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
     "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
 ]
@@ -52,7 +53,7 @@ class mhs_options(C.Structure):
                 ("max_levels", C.c_int), ("boundary_tol", C.c_double), ("boundary_max_cycles", C.c_int),
                 ("mu0", C.c_double), ("g", C.c_double),
                 ("p_b", C.POINTER(C.c_double)), ("rho_b", C.POINTER(C.c_double)), ("dfdz", C.POINTER(C.c_double)),
-                ("stream", C.c_void_p), ("profile", C.c_int), ("flags", C.c_int)]
+                ("stream", C.c_void_p), ("profile", C.c_int), ("flags", C.c_int), ("smoother", C.c_int), ("fmg_cycles", C.c_int)]
 
 
 class mhs_solve_info(C.Structure):
@@ -95,12 +96,13 @@ def lib():
         for n in ("mhs_solve_boundary", "mhs_solve_boundary_host"):
             getattr(L, n).argtypes = [vp, vp, C.POINTER(mhs_solve_info)]
         L.mhs_solve_interior.argtypes = [vp, dp, ip, C.POINTER(mhs_solve_info)]
+        L.mhs_solve_batch.argtypes = [vp, ip, vp, dp, ip, vp, vp, vp, vp, C.POINTER(mhs_solve_info)]
         for n in ("mhs_fields", "mhs_fields_host", "mhs_fields_host_async"):
             getattr(L, n).argtypes = [vp, vp, vp, vp]
         L.mhs_host_sync.argtypes = [vp]
         L.mhs_diagnostics.argtypes = [vp, vp, vp, vp, vp]
         L.mhs_fieldlines.argtypes = [vp, vp, ip, vp, dp, ip, ip, dp, vp, vp]
-        for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential"):
+        for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host"):
             getattr(L, n).argtypes = [vp, vp]
         L.mhs_last_error.argtypes = [vp]
         L.mhs_last_error.restype = C.c_char_p
@@ -161,7 +163,7 @@ def _info(i: mhs_solve_info, status):
 # ------------------------------------------------------------------ C-named functions ---------
 def mhs_create(nx, ny, nz, Lx, Ly, Lz, alpha, f_profile=None, *, dtype=torch.float64, omega=2.0 / 3.0,
                n_pre=2, n_post=2, max_levels=0, boundary_tol=1e-10, boundary_max_cycles=100, mu0=0.5, g=1.0,
-               p_b=None, rho_b=None, dfdz=None, stream=None, profile=0, flags=0):
+               p_b=None, rho_b=None, dfdz=None, stream=None, profile=0, flags=0, smoother=0, fmg_cycles=0):
     """-> opaque context handle (int).  See include/mhs.h: mhs_create."""
     L = lib()
     if not torch.cuda.is_available():
@@ -184,6 +186,7 @@ def mhs_create(nx, ny, nz, Lx, Ly, Lz, alpha, f_profile=None, *, dtype=torch.flo
     s = stream if stream is not None else torch.cuda.current_stream()
     o.stream = C.c_void_p(s.cuda_stream if hasattr(s, "cuda_stream") else int(s))
     o.profile, o.flags = profile, flags
+    o.smoother, o.fmg_cycles = smoother, fmg_cycles
     grid = mhs_grid(nx, ny, nz, Lx, Ly, Lz)
     h = C.c_void_p()
     st = L.mhs_create(C.byref(grid), alpha, keep[3].ctypes.data_as(pd) if keep[3] is not None else None,
@@ -293,6 +296,26 @@ class Solver:
     def solve_interior(self, tol=1e-10, max_cycles=100):
         return mhs_solve_interior(self.h, tol, max_cycles)
 
+    def solve_batch(self, Bz0, tol=1e-10, max_cycles=100, want=("P",)):
+        """mhs_solve_batch: Bz0 (nb, ny, nx) device tensor -> dict of outputs ("P" (nb, nz, ny, nx), "B" (nb, 3, nz, ny, nx),
+        "p", "rho") and the list of per-member interior-solve infos."""
+        nb = int(Bz0.shape[0])
+        shp = (self.nz, self.ny, self.nx)
+        mk = lambda *s: torch.empty(s, dtype=self.dtype, device="cuda")
+        out = {k: (mk(nb, 3, *shp) if k == "B" else mk(nb, *shp)) for k in want}
+        infos = (mhs_solve_info * max(nb, 1))()
+        ptr = lambda k, m: _dptr(out[k].reshape(-1), self.dtype, nb * m) if k in out else None
+        st = lib().mhs_solve_batch(self.h, nb, _dptr(Bz0.reshape(-1), self.dtype, nb * self.nx * self.ny), tol, max_cycles,
+                                   ptr("P", self.N), ptr("B", 3 * self.N), ptr("p", self.N), ptr("rho", self.N), infos)
+        _check(self.h, st, (MHS_ERR_NOT_CONVERGED,))
+        # (a member's own status: converged unless it used up max_cycles above the tolerance)
+        res = []
+        for b in range(nb):
+            i = infos[b]
+            ok = i.r_final <= tol * i.r0 or bool(i.stagnated)
+            res.append(_info(i, MHS_OK if ok else MHS_ERR_NOT_CONVERGED))
+        return out, res
+
     def host_sync(self):
         mhs_host_sync(self.h)
         self._inflight = []
@@ -340,6 +363,14 @@ class Solver:
         if out is None:
             out = torch.empty((self.nz, self.ny, self.nx), dtype=self.dtype, device="cuda")
         mhs_get_potential(self.h, out, self.dtype, self.N)
+        return out
+
+    def get_boundary(self, out=None, host=False):
+        """P(x, y, 0) of the last boundary solve, (ny, nx); host=True: into a pinned host tensor."""
+        if out is None:
+            out = torch.empty((self.ny, self.nx), dtype=self.dtype, device="cpu" if host else "cuda", pin_memory=host)
+        fn = lib().mhs_get_boundary_host if not out.is_cuda else lib().mhs_get_boundary
+        _check(self.h, fn(self.h, _dptr(out, self.dtype, self.nx * self.ny, "cuda" if out.is_cuda else "cpu")))
         return out
 
     def set_potential(self, P):

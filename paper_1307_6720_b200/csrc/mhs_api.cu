@@ -217,6 +217,21 @@ mhs_status build_hierarchy(mhs_ctx* ctx, int dim, std::vector<Level>& Ls)
         }
         mhs_status st = upload(ctx, &lv.tab, tab);
         if (st) return st;
+        if (dim == 3 && ctx->opt.smoother == MHS_SMOOTH_ZLINE && nz >= 3) {
+            // Thomas factors of the z-line matrix T = tridiag(a, D_k, a), a = 1/hz^2 (the same for every line; C25):
+            // den_k = D_k - a cp_{k-1}, cp_k = a / den_k;  the kernel multiplies by 1/den_k.
+            std::vector<double> zl(2 * (size_t)nz, 0.0);
+            const double a = 1.0 / (hz * hz);
+            double cprev = 0.0;
+            for (int k = 1; k <= nz - 2; ++k) {
+                const double den = tab[2 * (size_t)nz + k] - a * cprev;
+                if (!(den < 0.0)) return fail(ctx, MHS_ERR_INDEFINITE, "z-line matrix is not negative definite (alpha^2 too large)");
+                cprev = a / den;
+                zl[k] = cprev;
+                zl[(size_t)nz + k] = 1.0 / den;
+            }
+            if ((st = upload(ctx, &lv.zl, zl))) return st;
+        }
         if ((st = alloc_field(ctx, lv, 0, &lv.u))) return st;
         if (!(dim == 3 && l == 0))
             if ((st = alloc_field(ctx, lv, 2, &lv.rhs))) return st;
@@ -275,14 +290,18 @@ int kc_for(const Level& lv, int l, int what /*0 smooth 1 restrict 2 prolong 3 no
     return what;
 }
 
+// z-line Jacobi smoothing (mhs_options.smoother) applies to the 3D hierarchy
+bool use_zline(const mhs_ctx* ctx, const Level& lv) { return ctx->opt.smoother == MHS_SMOOTH_ZLINE && lv.dim == 3 && zline_ok(ctx, lv); }
+
 bool use_fast(const mhs_ctx* ctx, const Level& lv)
 {
-    return !(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fast_ok(ctx, lv);
+    return !(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fast_ok(ctx, lv) && &lv != ctx->ref_level;
 }
 
 bool use_zsweep(const mhs_ctx* ctx, const Level& lv)
 {
-    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && !mid_level(ctx, lv) && zsweep_ok(ctx, lv);
+    return !(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_UNFUSED_KERNELS)) && !mid_level(ctx, lv) && zsweep_ok(ctx, lv) &&
+           !(ctx->opt.smoother == MHS_SMOOTH_ZLINE && lv.dim == 3);
 }
 
 // residual + full weighting into co.rhs: separable form on big levels, register z-streaming on the others
@@ -304,6 +323,15 @@ long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const 
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
     const bool fast = use_fast(ctx, lv);
     long long npart = 0;
+    if (use_zline(ctx, lv)) {    // z-line Jacobi: one tridiagonal solve per (i,j) line and sweep (no norm by-product)
+        for (int s = 0; s < sweeps; ++s) {
+            Scope sc(ctx, kc_for(lv, l, 0));
+            launch_zline(ctx, lv, lv.u, rhs, lv.tmp, done);
+            std::swap(lv.u, lv.tmp);
+            if (lv.dim == 3 && l == 0) ctx->prof.sweeps_l0 += 1;
+        }
+        return 0;
+    }
     if (use_zsweep(ctx, lv)) {   // temporally blocked: two sweeps per pass over the iterate
         for (int s = 0; s < sweeps;) {
             const int S = std::min(2, sweeps - s);
@@ -350,11 +378,14 @@ void norm_final(mhs_ctx* ctx, const Level& lv, int l, long long n, int mode)
 // One V-cycle from level l (SURVEY 8(c) "V(u,rhs,l)").  Levels >= 1 start from u = 0.  At l == 0 with
 // fuse_norm the norm of the incoming iterate's residual is taken inside the first pre-sweep and the
 // stop rule (norm_final mode 1) is evaluated right after it, before the rest of the cycle is allowed to run.
-void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool fuse_norm = false)
+// cont (full-multigrid start, C26): level l >= 1 CONTINUES from the iterate in lv.u, whose bottom plane carries Dirichlet
+// data -- general kernels only on this level (no zero-guess shortcuts, not the cluster kernel, whose shared-memory levels
+// have zero walls); the levels below it are ordinary coarse-grid corrections.
+void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool fuse_norm = false, bool cont = false)
 {
     Level& lv = Ls[l];
     const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
-    if (l >= clus_of(ctx, Ls) && !lv.coarsest) {   // this level and everything below it: one cluster-kernel launch
+    if (l >= clus_of(ctx, Ls) && !lv.coarsest && !cont) {   // this level and everything below it: one cluster-kernel launch
         Scope sc(ctx, kc_for(lv, l, 0));
         launch_cluster(ctx, Ls, l, l == 0 ? 1 : 0, done);
         return;
@@ -368,9 +399,11 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
     const bool fast = use_fast(ctx, lv);
     int n_pre = ctx->opt.n_pre;
     const bool zs = use_zsweep(ctx, lv);
-    if (l > 0) {  // zero initial guess
+    if (l > 0 && !cont) {  // zero initial guess
         Scope sc(ctx, kc_for(lv, l, 0));
-        if (zs && n_pre >= 1) {
+        if (use_zline(ctx, lv)) {
+            cudaMemsetAsync(field_base(ctx, lv, lv.u), 0, (size_t)lv.alloc * ctx->es, ctx->stream);
+        } else if (zs && n_pre >= 1) {
             // the first sweep from zero is u = (omega/D) rhs: folded into the first temporally blocked pass
             const int S = std::min(2, n_pre);
             launch_zsweep(ctx, lv, nullptr, rhs, lv.u, S, true, false, done);
@@ -483,7 +516,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
         if ((h->cycles * (ctx->opt.n_pre + ctx->opt.n_post)) & 1) std::swap(l0.u, l0.tmp);
         return finish_cycles(ctx, tol, info);
     }
-    const bool fuse = use_fast(ctx, l0) && ctx->opt.n_pre >= 1 && !l0.coarsest && clus_of(ctx, Ls) > 0;
+    const bool fuse = use_fast(ctx, l0) && ctx->opt.n_pre >= 1 && !l0.coarsest && clus_of(ctx, Ls) > 0 && !use_zline(ctx, l0);
     std::vector<void*> iter_buf(1, l0.u);
     int issued = 0;
     bool trailing = false;
@@ -620,7 +653,8 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     if (bc && (bc->sides != MHS_BC_DIRICHLET_ZERO || bc->top != MHS_BC_DIRICHLET_ZERO))
         return fail(ctx, MHS_ERR_INVALID_ARG, "only MHS_BC_DIRICHLET_ZERO (P = 0 on sides and top, PAPER.md:96) is supported");
     if (!(o.omega > 0.0 && o.omega <= 1.0) || o.n_pre < 0 || o.n_post < 0 || o.n_pre + o.n_post < 1 || o.max_levels < 0 ||
-        !(o.mu0 > 0.0) || o.g == 0.0 || o.boundary_max_cycles < 1 || !(grid->Lx > 0 && grid->Ly > 0 && grid->Lz > 0))
+        !(o.mu0 > 0.0) || o.g == 0.0 || o.boundary_max_cycles < 1 || !(grid->Lx > 0 && grid->Ly > 0 && grid->Lz > 0) ||
+        (o.smoother != MHS_SMOOTH_JACOBI && o.smoother != MHS_SMOOTH_ZLINE) || o.fmg_cycles < 0)
         return fail(ctx, MHS_ERR_INVALID_ARG, "invalid option value");
     const int ext[3] = {grid->nx, grid->ny, grid->nz};
     const bool only2d = grid->nz == 1;   // boundary-only context: eq (11) on the plane, no interior (mhs.h, mhs_create)
@@ -673,9 +707,10 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ctx->debug = getenv("MHS_DEBUG") != nullptr;
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
-    ctx->tail3 = (ref || only2d) ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
+    const bool ref3 = ref || ctx->opt.smoother == MHS_SMOOTH_ZLINE;   // (the cluster kernel smooths with point Jacobi)
+    ctx->tail3 = (ref3 || only2d) ? (int)ctx->L3.size() : tail_start(ctx, ctx->L3, 216 * 1024);
     ctx->tail2 = ref ? (int)ctx->L2.size() : tail_start(ctx, ctx->L2, 216 * 1024);
-    ctx->clus3 = (ref || only2d) ? (int)ctx->L3.size() : cluster_start(ctx, ctx->L3, ctx->tail3);
+    ctx->clus3 = (ref3 || only2d) ? (int)ctx->L3.size() : cluster_start(ctx, ctx->L3, ctx->tail3);
     ctx->clus2 = ref ? (int)ctx->L2.size() : cluster_start(ctx, ctx->L2, ctx->tail2);
     if (!ref) ctx->cluster_max = cluster_max_size(ctx);
     ctx->npartial = std::max<long long>(64, resnorm_partial_capacity(ctx->L2[0]));
@@ -700,6 +735,7 @@ void mhs_destroy(mhs_ctx* ctx)
             for (void* p : lv.raw) if (p) cudaFree(p);
             if (lv.tab) cudaFree(lv.tab);
             if (lv.ainv) cudaFree(lv.ainv);
+            if (lv.zl) cudaFree(lv.zl);
         }
     if (ctx->prof_tab) cudaFree(ctx->prof_tab);
     if (ctx->partial) cudaFree(ctx->partial);
@@ -746,6 +782,7 @@ mhs_status mhs_solve_boundary(mhs_ctx* ctx, const void* Bz0, mhs_solve_info* inf
         CK(cudaMemcpyAsync(l3.tmp, ctx->L2[0].u, (size_t)l2.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
     }
     ctx->have_boundary = have3;
+    ctx->fmg_pending = have3;
     return st;
 }
 
@@ -759,6 +796,59 @@ mhs_status mhs_solve_boundary_host(mhs_ctx* ctx, const void* Bz0_host, mhs_solve
     return mhs_solve_boundary(ctx, ctx->bz_stage, info);
 }
 
+// Residual norm of the current level-0 iterate of a hierarchy, read back (one stream synchronisation).
+static mhs_status resnorm_now(mhs_ctx* ctx, std::vector<Level>& Ls, double* out)
+{
+    const long long np = resnorm_partials(ctx, Ls, 0, nullptr);
+    norm_final(ctx, Ls[0], 0, np, 2);
+    mhs_status rs = read_ctl(ctx);
+    if (rs) return rs;
+    drain_events(ctx);
+    *out = ctx->ctl_host->r_last;
+    return MHS_OK;
+}
+
+// Full-multigrid start (mhs_options.fmg_cycles; reading C26): replaces the interior of L3[0].u by the FMG iterate.
+// Level l carries the bottom data by injection; coarsest level: exact solve; level l < coarsest: trilinear interpolation
+// of the level below (whose bottom plane is then cleared again: below this point it only ever holds coarse-grid
+// corrections) + fmg_cycles V-cycles that continue from it.
+static mhs_status fmg_start(mhs_ctx* ctx)
+{
+    std::vector<Level>& Ls = ctx->L3;
+    const int n = (int)Ls.size();
+    Scope sc(ctx, MHS_KC_COARSE_3D);
+    for (int l = 1; l < n; ++l) {
+        Level& lv = Ls[l];
+        CK(cudaMemsetAsync(field_base(ctx, lv, lv.u), 0, (size_t)lv.alloc * ctx->es, ctx->stream));
+        if (lv.tmp) CK(cudaMemsetAsync(field_base(ctx, lv, lv.tmp), 0, (size_t)lv.alloc * ctx->es, ctx->stream));
+        CK(cudaMemsetAsync(field_base(ctx, lv, lv.rhs), 0, (size_t)lv.alloc * ctx->es, ctx->stream));
+        launch_inject_bottom(ctx, Ls[0], Ls[0].u, lv, 1 << l, lv.u, lv.tmp);
+    }
+    {
+        Level& lc = Ls[n - 1];
+        launch_bottom_rhs(ctx, lc, lc.u, lc.rhs);
+        launch_coarse_solve(ctx, lc, lc.u, lc.rhs, nullptr);
+        CK(cudaMemsetAsync(field_base(ctx, lc, lc.rhs), 0, (size_t)lc.alloc * ctx->es, ctx->stream));
+    }
+    for (int l = n - 2; l >= 0; --l) {
+        Level& lv = Ls[l];
+        Level& co = Ls[l + 1];
+        // interior <- 0 (planes 1 .. of both buffers' current iterate), then u += P u_coarse: the interpolation itself
+        CK(cudaMemsetAsync((char*)lv.u + (size_t)lv.sp * ctx->es, 0, (size_t)lv.sp * (lv.nz - 1) * ctx->es, ctx->stream));
+        if (use_fast(ctx, lv)) launch_prolong_v(ctx, lv, lv.u, co, co.u, 0, nullptr);
+        else launch_prolong_ref(ctx, lv, lv.u, co, co.u, nullptr);
+        // the level below goes back to zero walls
+        CK(cudaMemsetAsync(co.u, 0, (size_t)co.sp * ctx->es, ctx->stream));
+        if (co.tmp) CK(cudaMemsetAsync(co.tmp, 0, (size_t)co.sp * ctx->es, ctx->stream));
+        // (levels the cluster kernel normally runs are tiny: the one-thread-per-node kernels serve them here)
+        if (l > 0 && l >= ctx->clus3) ctx->ref_level = &lv;
+        for (int q = 0; q < ctx->opt.fmg_cycles; ++q) vcycle(ctx, Ls, l, nullptr, false, l > 0);
+        ctx->ref_level = nullptr;
+    }
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
 mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solve_info* info)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
@@ -767,12 +857,55 @@ mhs_status mhs_solve_interior(mhs_ctx* ctx, double tol, int max_cycles, mhs_solv
     if (!ctx->have_boundary) return fail(ctx, MHS_ERR_STATE, "mhs_solve_interior before a successful mhs_solve_boundary / mhs_set_potential");
     mhs_solve_info local;
     if (!info) info = &local;
+    if (ctx->opt.fmg_cycles > 0 && ctx->fmg_pending) {
+        ctx->fmg_pending = false;
+        // r0 is the residual norm of the iterate the solve starts from by the paper's procedure (zero interior),
+        // taken before the full-multigrid start replaces that interior
+        double r0 = 0.0, r1 = 0.0;
+        mhs_status fs = resnorm_now(ctx, ctx->L3, &r0);
+        if (fs) return fs;
+        if ((fs = fmg_start(ctx))) return fs;
+        if ((fs = resnorm_now(ctx, ctx->L3, &r1))) return fs;
+        ctx->have_r0 = r0 > 0.0;
+        ctx->r0_interior = r0;
+        if (!(r1 == r1) || std::isinf(r1)) return fail(ctx, MHS_ERR_INDEFINITE, "residual norm is not finite after the full-multigrid start");
+        if (r1 <= tol * r0) {   // the FMG iterate already meets the tolerance: no ordinary cycle
+            memset(info, 0, sizeof *info);
+            info->r0 = r0; info->r_final = r1;
+            return MHS_OK;
+        }
+    }
     mhs_status st = run_cycles(ctx, ctx->L3, tol, max_cycles, ctx->have_r0 ? ctx->r0_interior : 0.0, info);
+    ctx->fmg_pending = false;
     if (st == MHS_OK || st == MHS_ERR_NOT_CONVERGED) {
         ctx->have_r0 = info->r0 > 0.0;
         ctx->r0_interior = info->r0;
     }
     return st;
+}
+
+mhs_status mhs_solve_batch(mhs_ctx* ctx, int nb, const void* Bz0, double tol, int max_cycles, void* P, void* B, void* p, void* rho,
+                           mhs_solve_info* infos)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L3.empty()) return fail(ctx, MHS_ERR_STATE, "this context has no 3D grid (nz = 1: boundary solve only)");
+    if (nb < 0 || (nb > 0 && !Bz0)) return fail(ctx, MHS_ERR_INVALID_ARG, "nb must be >= 0 and Bz0 non-NULL");
+    const size_t es = (size_t)ctx->es, n2 = (size_t)ctx->grid.nx * ctx->grid.ny, N = (size_t)ctx->L3[0].npts();
+    bool all_converged = true;
+    for (int b = 0; b < nb; ++b) {
+        mhs_status st = mhs_solve_boundary(ctx, (const char*)Bz0 + (size_t)b * n2 * es, nullptr);
+        if (st != MHS_OK && st != MHS_ERR_NOT_CONVERGED) return st;
+        st = mhs_solve_interior(ctx, tol, max_cycles, infos ? infos + b : nullptr);
+        if (st == MHS_ERR_NOT_CONVERGED) all_converged = false;
+        else if (st != MHS_OK) return st;
+        if (P && (st = mhs_get_potential(ctx, (char*)P + (size_t)b * N * es))) return st;
+        if (B || p || rho)
+            if ((st = mhs_fields(ctx, B ? (char*)B + (size_t)b * 3 * N * es : nullptr, p ? (char*)p + (size_t)b * N * es : nullptr,
+                                 rho ? (char*)rho + (size_t)b * N * es : nullptr)))
+                return st;
+    }
+    if (!all_converged) return fail(ctx, MHS_ERR_NOT_CONVERGED, "max_cycles reached before the tolerance for at least one member of the batch");
+    return MHS_OK;
 }
 
 mhs_status mhs_get_potential(mhs_ctx* ctx, void* P)
@@ -801,6 +934,31 @@ mhs_status mhs_get_potential_host(mhs_ctx* ctx, void* P_host)
     return MHS_OK;
 }
 
+mhs_status mhs_get_boundary(mhs_ctx* ctx, void* P0)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L2.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    if (!P0) return fail(ctx, MHS_ERR_INVALID_ARG, "P0 is NULL");
+    Scope sc(ctx, MHS_KC_PACK);
+    launch_unpack(ctx, ctx->L2[0], ctx->L2[0].u, P0);
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_get_boundary_host(mhs_ctx* ctx, void* P0_host)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (ctx->L2.empty()) return fail(ctx, MHS_ERR_STATE, "context was not created successfully");
+    if (!P0_host) return fail(ctx, MHS_ERR_INVALID_ARG, "P0 is NULL");
+    // (the magnetogram's device copy has been consumed by the solve: it serves as the dense staging plane)
+    const size_t bytes = (size_t)ctx->grid.nx * ctx->grid.ny * ctx->es;
+    mhs_status st = mhs_get_boundary(ctx, ctx->bz_stage);
+    if (st) return st;
+    CK(cudaMemcpyAsync(P0_host, ctx->bz_stage, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return MHS_OK;
+}
+
 mhs_status mhs_set_potential(mhs_ctx* ctx, const void* P)
 {
     if (!ctx) return MHS_ERR_INVALID_ARG;
@@ -813,6 +971,7 @@ mhs_status mhs_set_potential(mhs_ctx* ctx, const void* P)
     CK(cudaGetLastError());
     ctx->have_boundary = true;
     ctx->have_r0 = false;
+    ctx->fmg_pending = false;   // (a potential given by the caller is continued from, never replaced)
     return MHS_OK;
 }
 
@@ -970,6 +1129,7 @@ mhs_status mhs_level_set(mhs_ctx* ctx, int dim, int level, int which, const void
     if (bottom) {
         CK(cudaMemcpyAsync(lv.tmp, lv.u, (size_t)lv.sp * ctx->es, cudaMemcpyDeviceToDevice, ctx->stream));
         ctx->have_r0 = false;
+        ctx->fmg_pending = false;
         ctx->have_boundary = true;   // (the same as mhs_set_potential)
     }
     CK(cudaGetLastError());

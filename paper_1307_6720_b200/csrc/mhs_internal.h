@@ -52,6 +52,7 @@ struct Level {
     std::vector<double> c;  // 1 + f at this level's planes
     int ncoarse = 0;        // unknowns of the exact solve (coarsest level only)
     void* ainv = nullptr;   // device T[ncoarse^2]
+    void* zl = nullptr;     // device T[2*nz]: Thomas factors cp | 1/den of the z-line smoother (mhs_options.smoother = 1)
     long long npts() const { return (long long)nx * ny * nz; }
 };
 
@@ -79,6 +80,8 @@ struct mhs_ctx {
     cudaEvent_t ev_fields = nullptr, ev_copied = nullptr;
     bool copy_pending = false;
     bool have_boundary = false, have_r0 = false;
+    bool fmg_pending = false;          // mhs_solve_boundary has run and no interior cycle yet: the FMG start may replace the interior
+    const mhs::Level* ref_level = nullptr;   // a level that must run the general reference kernels right now (FMG start)
     double r0_interior = 0;
     mhs_profile prof{};
     int cur_kc = MHS_KC_PACK;  // kernel class the launchers charge
@@ -159,6 +162,11 @@ void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void
 bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
 void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ);
+// ---- solver variants (mhs_kernels_variants.cu): z-line Jacobi, full-multigrid start ----
+bool zline_ok(const mhs_ctx* c, const Level& lv);
+void launch_zline(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done);
+void launch_inject_bottom(mhs_ctx* c, const Level& fine, const void* fine_u, const Level& lv, int stride, void* a, void* b);
+void launch_bottom_rhs(mhs_ctx* c, const Level& lv, const void* u, void* rhs);
 // ---- field-line integration (mhs_kernels_lines.cu) ----
 void launch_fieldlines(mhs_ctx* c, const Level& lv, const void* B, int nseeds, const void* seeds, double step, int max_points, int direction,
                        double bmin, void* lines, int* npoints);

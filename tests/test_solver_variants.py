@@ -201,3 +201,218 @@ def test_jacobi_weight_six_sevenths_is_the_better_3d_smoother(orc):
     _, a = orc.solve_interior(P, w.f, w.alpha, w.L, omega=2.0 / 3.0)
     _, b = orc.solve_interior(P, w.f, w.alpha, w.L, omega=6.0 / 7.0)
     assert b["cycles"] <= a["cycles"]
+
+
+# ====================================================================== GPU parity ======================
+def _B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1307_6720_b200 import binding
+    binding.lib()
+    return binding, torch
+
+
+def _dev(a, dtype):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device="cuda").contiguous()
+
+
+def _host(t):
+    return t.detach().cpu().double().numpy()
+
+
+def _relmax(a, b):
+    s = np.abs(b).max()
+    return np.abs(a - b).max() / (s if s > 0 else 1.0)
+
+
+def _aniso(n=65):
+    """1 - xi from 0.05 at the base to 0.65 at the top (the regime of the paper's xi_2) on the config-1 sources."""
+    w = inputs.config(1, shrink=128 // (n - 1))
+    w.f = -(0.95 * np.exp(-1.0 * np.linspace(0.0, w.Lz, w.nz)))
+    w.name = "aniso%d" % n
+    return w
+
+
+VW = {
+    "ragged_17x33x9": lambda: inputs.small(),
+    "cfg0_33": lambda: inputs.config(0),
+    "cfg1_65": lambda: inputs.config(1, shrink=2),
+    "aniso_65": lambda: _aniso(65),
+    "cfg1_129": lambda: inputs.config(1),
+    "cfg4_129x129x33": lambda: inputs.config(4, shrink=8),
+}
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype_name", ["f64", "f32"])
+@pytest.mark.parametrize("sweeps", [(2, 2), (1, 1), (2, 1)])
+@pytest.mark.parametrize("name", ["ragged_17x33x9", "cfg0_33", "aniso_65", "cfg4_129x129x33"])
+def test_zline_per_iterate_parity(orc, name, sweeps, dtype_name):
+    """mhs_options.smoother = MHS_SMOOTH_ZLINE: single sweeps (levels 0 and 1, with a right-hand side on level 1) and eight
+    V-cycle iterates against the oracle, 1e-12 (fp64) / 1e-5 (fp32) per iterate."""
+    B, torch = _B()
+    dtype = torch.float64 if dtype_name == "f64" else torch.float32
+    tol = 1e-12 if dtype_name == "f64" else 1e-5
+    optol = 1e-13 if dtype_name == "f64" else 2e-6
+    w = VW[name]()
+    a, b = sweeps
+    c = 1.0 + w.f
+    omega = 0.8
+    with B.Solver.from_workload(w, dtype=dtype, n_pre=a, n_post=b, omega=omega, smoother=B.MHS_SMOOTH_ZLINE,
+                                boundary_tol=1e-10 if dtype_name == "f64" else 1e-6) as S:
+        if sweeps == (2, 2):
+            for lvl in (0, 1):
+                shp = S._shape(3, lvl)
+                u = inputs.random_field(shp, 700 + lvl)
+                rhs = None
+                if lvl == 0:
+                    u[0] = inputs.random_field(shp[1:], 710)
+                else:
+                    rhs = inputs.random_field(shp, 720)
+                    S.level_set(3, lvl, 1, _dev(rhs, dtype))
+                S.level_set(3, lvl, 0, _dev(u, dtype))
+                S.op_smooth(3, lvl, 1)
+                Ll = w.L
+                ref = orc.zline3(u, rhs, c[:: 2**lvl], w.alpha, omega, Ll)
+                assert _relmax(_host(S.level_get(3, lvl, 0)), ref) <= 4 * optol, lvl
+        S.solve_boundary(_dev(w.Bz0, dtype))
+        P = _host(S.get_potential())
+        r0 = orc.resnorm3(P, None, c, w.alpha, w.L)
+        for k in range(8):
+            info = S.solve_interior(0.0, 1)
+            P = orc.vcycle3s(P, None, c, w.alpha, w.L, omega=omega, n_pre=a, n_post=b, smoother=1)
+            err = _relmax(_host(S.get_potential()), P)
+            assert err <= tol, (name, sweeps, k, err)
+            rk = orc.resnorm3(P, None, c, w.alpha, w.L)
+            if rk / r0 > (1e-4 if dtype_name == "f32" else 1e-8):
+                assert abs(info["history"][0] - rk) <= (1e-2 if dtype_name == "f32" else 1e-6) * rk
+
+
+@pytest.mark.gpu
+def test_zline_solve_to_tolerance_and_cycle_savings(orc):
+    """One call to 1e-10 with z-line smoothing on the strongly anisotropic problem: the oracle's cycle count and solution,
+    three times fewer cycles than point Jacobi needs on the same problem."""
+    B, torch = _B()
+    w = _aniso(65)
+    with B.Solver.from_workload(w, omega=0.8, smoother=B.MHS_SMOOTH_ZLINE) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        P0 = _host(S.get_potential())
+        iz = S.solve_interior(1e-10, 200)
+        Po, oi = orc.solve_interior_opt(P0, w.f, w.alpha, w.L, omega=0.8, smoother=1, tol=1e-10, max_cycles=200)
+        assert iz["converged"] and iz["cycles"] == oi["cycles"]
+        assert _relmax(_host(S.get_potential()), Po) <= 1e-12
+    with B.Solver.from_workload(w) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        ip = S.solve_interior(1e-10, 200)
+        assert ip["converged"] and ip["cycles"] >= 3 * iz["cycles"], (ip["cycles"], iz["cycles"])
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("flags", [0, 8])
+@pytest.mark.parametrize("smoother,nfmg", [(0, 1), (0, 2), (1, 1)])
+@pytest.mark.parametrize("name", ["ragged_17x33x9", "cfg0_33", "cfg1_65", "cfg1_129", "cfg4_129x129x33"])
+def test_fmg_start_parity(orc, name, smoother, nfmg, flags):
+    """mhs_options.fmg_cycles: (i) the full-multigrid iterate itself (a call whose tolerance it meets returns 0 cycles),
+    (ii) the solve to tolerance -- r0, cycle count, solution -- against orc_solve_interior_opt."""
+    B, torch = _B()
+    w = VW[name]()
+    omega = 0.8 if smoother else w.omega
+    kw = dict(omega=omega, smoother=smoother, fmg_cycles=nfmg, flags=flags, dtype=torch.float64)
+    with B.Solver.from_workload(w, **kw) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        P0 = _host(S.get_potential())
+        i0 = S.solve_interior(1e30, 5)                      # any iterate meets this tolerance: FMG start only
+        assert i0["cycles"] == 0 and i0["converged"]
+        guess = orc.fmg_interior(P0, w.f, w.alpha, w.L, omega=omega, n_pre=w.n_pre, n_post=w.n_post, smoother=smoother, n_fmg=nfmg)
+        assert _relmax(_host(S.get_potential()), guess) <= 1e-12
+        c = 1.0 + w.f
+        assert abs(i0["r0"] - orc.resnorm3(P0, None, c, w.alpha, w.L)) <= 1e-9 * i0["r0"]
+        assert abs(i0["r_final"] - orc.resnorm3(guess, None, c, w.alpha, w.L)) <= 1e-6 * i0["r_final"]
+        # a second call continues from the FMG iterate with ordinary cycles (no second FMG start)
+        i1 = S.solve_interior(0.0, 1)
+        P1 = orc.vcycle3s(guess, None, c, w.alpha, w.L, omega=omega, n_pre=w.n_pre, n_post=w.n_post, smoother=smoother)
+        assert i1["cycles"] == 1 and _relmax(_host(S.get_potential()), P1) <= 1e-12
+    with B.Solver.from_workload(w, **kw) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        info = S.solve_interior(w.tol, 100)
+        Po, oi = orc.solve_interior_opt(P0, w.f, w.alpha, w.L, omega=omega, n_pre=w.n_pre, n_post=w.n_post, smoother=smoother,
+                                        fmg=nfmg, tol=w.tol)
+        assert info["converged"] and info["cycles"] == oi["cycles"], (info["cycles"], oi["cycles"])
+        assert abs(info["r0"] - oi["r0"]) <= 1e-9 * oi["r0"]
+        assert _relmax(_host(S.get_potential()), Po) <= 1e-12
+        # mhs_set_potential is continued from, never replaced by an FMG start
+        S.set_potential(_dev(P0, torch.float64))
+        i2 = S.solve_interior(0.0, 1)
+        P2 = orc.vcycle3s(P0, None, 1.0 + w.f, w.alpha, w.L, omega=omega, n_pre=w.n_pre, n_post=w.n_post, smoother=smoother)
+        assert _relmax(_host(S.get_potential()), P2) <= 1e-12
+
+
+@pytest.mark.gpu
+def test_fmg_saves_cycles_at_full_size(orc):
+    """BASELINE configs[2] (257^3): with a one-cycle-per-level FMG start the solve to 1e-10 needs fewer finest-level cycles
+    and reaches the same potential; the FMG iterate is checked against the oracle (~1.5 V-cycles of oracle work)."""
+    B, torch = _B()
+    w = inputs.config(2)
+    with B.Solver.from_workload(w) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        P0 = _host(S.get_potential())
+        ia = S.solve_interior(w.tol, 100)
+        Pa = S.get_potential().clone()
+    with B.Solver.from_workload(w, fmg_cycles=1) as S:
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        i0 = S.solve_interior(1e30, 1)
+        guess = orc.fmg_interior(P0, w.f, w.alpha, w.L)
+        assert i0["cycles"] == 0 and _relmax(_host(S.get_potential()), guess) <= 1e-12
+        S.solve_boundary(_dev(w.Bz0, torch.float64))
+        ib = S.solve_interior(w.tol, 100)
+        assert ib["converged"] and ib["cycles"] <= ia["cycles"] - 3, (ia["cycles"], ib["cycles"])
+        assert abs(ib["r0"] - ia["r0"]) <= 1e-12 * ia["r0"]
+        assert float((S.get_potential() - Pa).abs().max()) <= 1e-8 * float(Pa.abs().max())
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cfg0_33", "ragged_17x33x9", "cfg1_65"])
+def test_jacobi_weight_option_parity(orc, name):
+    """omega = 6/7 (the 3D smoothing-optimal Jacobi weight; C4 makes omega an option) through every kernel family."""
+    B, torch = _B()
+    w = VW[name]()
+    om = 6.0 / 7.0
+    for flags in (0, 8, 1):
+        with B.Solver.from_workload(w, omega=om, flags=flags) as S:
+            S.solve_boundary(_dev(w.Bz0, torch.float64))
+            P = _host(S.get_potential())
+            c = 1.0 + w.f
+            for k in range(5):
+                S.solve_interior(0.0, 1)
+                P = orc.vcycle3(P, None, c, w.alpha, w.L, omega=om, n_pre=w.n_pre, n_post=w.n_post)
+                assert _relmax(_host(S.get_potential()), P) <= 1e-12, (flags, k)
+
+
+@pytest.mark.gpu
+def test_solve_batch_equals_member_by_member(orc):
+    """mhs_solve_batch on three magnetograms of one region: every member equals, bit for bit, what the separate calls give,
+    and the oracle's solve of that member; infos carry each member's cycle count."""
+    B, torch = _B()
+    ws = [inputs.config(1, shrink=2, replica=r) for r in range(3)]
+    w = ws[0]
+    bz = torch.stack([_dev(x.Bz0, torch.float64) for x in ws])
+    with B.Solver.from_workload(w) as S:
+        out, infos = S.solve_batch(bz, w.tol, 100, want=("P", "B", "rho"))
+        for b, x in enumerate(ws):
+            S.solve_boundary(_dev(x.Bz0, torch.float64))
+            i = S.solve_interior(w.tol, 100)
+            assert i["cycles"] == infos[b]["cycles"] and infos[b]["converged"]
+            assert torch.equal(S.get_potential(), out["P"][b])
+            Bf, _, rho = S.fields(want=("B", "rho"))
+            assert torch.equal(Bf, out["B"][b]) and torch.equal(rho, out["rho"][b])
+            P0, _ = orc.solve_boundary(x.Bz0, (w.Lx, w.Ly))
+            Po = np.zeros(w.shape); Po[0] = P0
+            Po, oi = orc.solve_interior(Po, w.f, w.alpha, w.L)
+            assert oi["cycles"] == infos[b]["cycles"] and _relmax(_host(out["P"][b]), Po) <= 1e-12
+        # max_cycles too small for every member: reported, results are the valid 2nd iterates
+        out2, infos2 = S.solve_batch(bz, w.tol, 2, want=("P",))
+        assert all(i["cycles"] == 2 and not i["converged"] for i in infos2)
+        empty, none = S.solve_batch(bz[:0], w.tol, 5)
+        assert none == [] and empty["P"].shape[0] == 0
