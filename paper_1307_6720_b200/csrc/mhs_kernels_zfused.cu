@@ -166,14 +166,16 @@ __device__ __forceinline__ double zc_iw2(const ZCoef<float>&) { return 0.0; }
 // One Jacobi update of one row of a thread's patch.  c: the row's centre values, w/e: the elements left / right of
 // the vector, n/s: the rows above / below, up/dn: the planes above / below, f: right-hand side.  rs (fp32 only): the
 // sum of the squared residuals of the row, without element 0 when it is a wall (cw0).
-template <bool HAS_RHS>
+// ISO: hx == hy, i.e. rho == 1: fma(1, a, b) is a + b rounded once, so the plain sum gives the same bits with one fp64
+// instruction less per update (6 instead of 7) -- the fp64 pipe is the kernel's second busiest unit.
+template <bool HAS_RHS, bool ISO>
 __device__ __forceinline__ void jac_row(const ZCoef<double>& k, double rho, double, double, const ZVec<double>& c, double w, double e,
                                         const ZVec<double>& n, const ZVec<double>& s, const ZVec<double>& up, const ZVec<double>& dn,
                                         const ZVec<double>& f, ZVec<double>& o, bool, float&)
 {
     double o0 = k.A * c.v[0], o1 = k.A * c.v[1];
-    const double h0 = fma(rho, c.v[1] + w, n.v[0] + s.v[0]);
-    const double h1 = fma(rho, e + c.v[0], n.v[1] + s.v[1]);
+    const double h0 = ISO ? (c.v[1] + w) + (n.v[0] + s.v[0]) : fma(rho, c.v[1] + w, n.v[0] + s.v[0]);
+    const double h1 = ISO ? (e + c.v[0]) + (n.v[1] + s.v[1]) : fma(rho, e + c.v[0], n.v[1] + s.v[1]);
     o0 = fma(k.By, h0, o0);
     o1 = fma(k.By, h1, o1);
     o0 = fma(k.Bz, up.v[0] + dn.v[0], o0);
@@ -186,7 +188,7 @@ __device__ __forceinline__ void jac_row(const ZCoef<double>& k, double rho, doub
     o.v[1] = o1;
 }
 
-template <bool HAS_RHS>
+template <bool HAS_RHS, bool ISO>
 __device__ __forceinline__ void jac_row(const ZCoef<float>& k, float, float cz, float a2, const ZVec<float>& c, float w, float e,
                                         const ZVec<float>& n, const ZVec<float>& s, const ZVec<float>& up, const ZVec<float>& dn,
                                         const ZVec<float>& f, ZVec<float>& o, bool cw0, float& rs)
@@ -470,7 +472,7 @@ __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* til
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (steps come in pairs).
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO, bool ISO>
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
 {
@@ -548,7 +550,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             const ZVec<T> ss = r == 0 ? in.edge1 : c0.r[r > 0 ? r - 1 : 0];
             float rs = 0.f;
             const T w1 = z.swp ? in.e : in.w, e1 = z.swp ? in.w : in.e;
-            jac_row<HAS_RHS>(k1, p.rho, p.cz, p.a2, c0.r[r], w1, e1, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
+            jac_row<HAS_RHS, ISO>(k1, p.rho, p.cz, p.a2, c0.r[r], w1, e1, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
             if (z.cw0) o1.v[0] = c0.r[r].v[0];
             if (NORM && (m1 & (1 << r))) {
                 if (sizeof(T) == 8) {
@@ -573,7 +575,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             const ZVec<T> ss = r == 0 ? in.edge2 : c1.r[r > 0 ? r - 1 : 0];
             float rs;
             const T w2 = z.swp ? in.e2 : in.w2, e2 = z.swp ? in.w2 : in.e2;
-            jac_row<HAS_RHS>(k2, p.rho, p.cz, p.a2, c1.r[r], w2, e2, nn, ss, o1, dn1.r[r], in.f2, o2, false, rs);
+            jac_row<HAS_RHS, ISO>(k2, p.rho, p.cz, p.a2, c1.r[r], w2, e2, nn, ss, o1, dn1.r[r], in.f2, o2, false, rs);
             if (z.cw0) o2.v[0] = c1.r[r].v[0];
             if (m2 & (1 << r)) zst(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
@@ -589,7 +591,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     z_advance<T, WXT, ZERO, PRO>(p, z, tile_src, IN, true);
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO, bool ISO>
 __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
 {
@@ -734,8 +736,8 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
         // (no moves).  An odd segment runs one idle step past its end: nothing arrives, nothing is stored (masks),
         // the coefficient table has a spare record for it.
         do {
-            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>(p, z, tile_src, IN, Y, X, Q, P);
-            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>(p, z, tile_src, IN, X, Y, P, Q);
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO, ISO>(p, z, tile_src, IN, Y, X, Q, P);
+            z_step<T, WXT, S, HAS_RHS, ZERO, NORM, PRO, ISO>(p, z, tile_src, IN, X, Y, P, Q);
         } while (z.t <= tend);
         // planes requested but not consumed cannot exist (requests stop at kend_in, steps run past it)
     }
@@ -809,11 +811,15 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro =
     return z;
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO = false>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO = false, bool ISO = false>
 static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done,
                            const void* ec = nullptr, long long csp = 0)
 {
-    auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM, PRO>;
+    // the isotropic specialisation exists for the fp64 passes of the finest level (no right-hand side), where the time goes
+    if constexpr (!ISO && !HAS_RHS && !ZERO && sizeof(T) == 8) {
+        if (lv.hx == lv.hy) return zsweep_launch_w<T, WXT, S, HAS_RHS, ZERO, NORM, PRO, true>(c, lv, z, u, rhs, out, done, ec, csp);
+    }
+    auto kern = k_zsweep<T, WXT, S, HAS_RHS, ZERO, NORM, PRO, ISO>;
     static PerDevice attr;
     per_device(attr, c, [&] {
         cudaFuncAttributes fa;
@@ -839,8 +845,8 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZV<T>::WY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (c->debug) {
         cudaError_t e = cudaPeekAtLastError();
-        fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
-                sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, (int)PRO, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
+        fprintf(stderr, "[mhs] k_zsweep<%s,WX=%d,S=%d,rhs=%d,zero=%d,norm=%d,pro=%d,iso=%d> %dx%dx%d TC %d ntx %d nty %d ctas %d smem %zu: %s\n",
+                sizeof(T) == 8 ? "f64" : "f32", WXT, S, (int)HAS_RHS, (int)ZERO, (int)NORM, (int)PRO, (int)ISO, lv.nx, lv.ny, lv.nz, z.TC, z.ntx, z.nty,
                 z.ctas, z.smem, cudaGetErrorString(e));
     }
     return z.ctas;
