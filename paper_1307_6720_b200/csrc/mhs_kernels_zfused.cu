@@ -25,9 +25,13 @@
 //   * The squared norm of the residual of the INPUT iterate is a by-product of stage 1 (r = (u'-u) D/w).
 //   * Work is a linearised list of (tile, plane) pairs cut into equal contiguous ranges, one per CTA, one CTA
 //     per SM: no wave quantisation whatever the grid size.
+#include <algorithm>
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <map>
+#include <mutex>
+#include <tuple>
 
 #include "mhs_device.cuh"
 
@@ -54,6 +58,7 @@ template <typename T, int WXT> struct ZG {
     static constexpr int CROWS = ZWY * ZR / 2 + 2;
     static constexpr int CINP = CROWS * CSX + 16 / (int)sizeof(T);   // + the element after the last row (16-byte granule)
 };
+constexpr int ZQB = 200;   // capacity of the work partition table: at most ZQB-1 CTAs
 constexpr int ZNIN = 4;   // input ring depth (planes); 3 in the prolongation-fused variant (shared memory pays for the coarse ring)
 constexpr int ZNCE = 3;   // coarse-correction ring depth (planes), prolongation-fused variant only
 
@@ -86,6 +91,7 @@ struct ZP {
     long long csp;      //   its plane stride
     int in_plane;       // elements of one ring slot: (WY*ZR + 2) rows x TC (also the size of an exchange plane)
     int coef_bytes;     // bytes reserved for the coefficient table (multiple of 128)
+    int qb[ZQB];        // CTA b works on the items [qb[b], qb[b+1]) of the linearised (tile, plane) list (zpartition)
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -283,7 +289,10 @@ struct ZCtx {
     uint32_t in_base, ce_base;    // shared-space addresses of ring slot 0 / coarse ring slot 0
     uint32_t ce_own;              // byte offset, inside a coarse slot, of (coarse row jrow0>>1, coarse column of element 0)
     int czoff, cnext;             // ring position of coarse plane K is czoff + K; next coarse plane to request
-    int jt, Jb;                   // first patch row of the tile; first coarse row held in a coarse slot
+    int jt, Jb;                   // first patch row of the tile (always odd); first coarse row held in a coarse slot
+    uint32_t c0a, c1a;            // this step's two coarse planes (shared-space addresses), set by z_prolong
+    bool corr;                    // the plane that arrives in this step takes a correction (interior plane)
+    bool wrow;                    // the last patch row of this thread is the wall row j = sy (last tile along y): held at zero
 };
 
 // warp 0: request input plane `k` of the tile into ring slot nload % NIN
@@ -411,8 +420,8 @@ __device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, 
     }
 }
 
-template <typename T, int WXT, int NIN>
-__device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int t, int slot)
+template <typename T, int WXT, int NIN, bool ROWS = true>
+__device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int slot)
 {
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N, VC = V / 2;
@@ -420,15 +429,17 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, const ZCtx<T>& z, int 
     constexpr int TC = ZG<T, WXT>::TC, NR = ZWY * ZR;
     constexpr uint32_t planeb = (uint32_t)ZG<T, WXT>::INP * ES, cplaneb = (uint32_t)ZG<T, WXT>::CINP * ES;
     constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
+    z.corr = false;
     if (t < 1 || t > p.nz - 2) return;
+    z.corr = true;
     const int K0 = t >> 1, K1 = (t + 1) >> 1;
     const int p0 = z.czoff + K0, p1 = z.czoff + K1;
     mbar_wait32(z.bars + 8 * (NIN + p0 % ZNCE), (uint32_t)((p0 / ZNCE) & 1));
     mbar_wait32(z.bars + 8 * (NIN + p1 % ZNCE), (uint32_t)((p1 / ZNCE) & 1));
     const uint32_t c0a = z.ce_base + (uint32_t)(p0 % ZNCE) * cplaneb, c1a = z.ce_base + (uint32_t)(p1 % ZNCE) * cplaneb;
     const uint32_t a_pl = z.in_own + (uint32_t)slot * planeb;
-    if (z.jt & 1) z_prolong_rows<T, WXT, 1>(z, a_pl, c0a, c1a);     // (patch rows start ZR-aligned from jt: same parity)
-    else z_prolong_rows<T, WXT, 0>(z, a_pl, c0a, c1a);
+    z.c0a = c0a; z.c1a = c1a;
+    if (ROWS) z_prolong_rows<T, WXT, 1>(z, a_pl, c0a, c1a);     // (jt is odd and patch rows start ZR-aligned from it)
     // the halo rows of the tile (fine rows jt-1 and jt+NR): one vector per thread
     const int nvr = TC / V;
     const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
@@ -469,6 +480,135 @@ __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* til
     z_advance<T, WXT, ZERO, PRO>(p, z, tile_src, IN, false);
 }
 
+// pa += d0^2 + d1^2 where `on` is set: predicated FMAs (written as a select ptxas makes 2 FSEL per value of them)
+__device__ __forceinline__ void norm_acc(double& pa, double d0, double d1, int on)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p fma.rn.f64 %0, %1, %1, %0;\n\t@p fma.rn.f64 %0, %2, %2, %0;\n\t}"
+        : "+d"(pa)
+        : "d"(d0), "d"(d1), "r"(on));
+}
+
+// The rows of one plane step in fp64 (not the zero-guess variant).  The update is evaluated as
+//     u' = [A c + By h + Bz dn (+ wz f)] + Bz up,        h = rho (e + w) + (n + s)
+// i.e. everything but the last FMA is independent of the plane that arrives in this step (stage 1) and of the sweep-1
+// value made in this step (stage 2).  Two things follow.  (i) The bracket of row r+1 is formed while row r is finished, so
+// the shared-memory round trip of `up` and the stage 1 -> stage 2 dependency each cost one FMA of latency instead of an
+// add + an FMA.  (ii) `dn` is dead once the bracket exists: the arriving plane is loaded straight into the registers of dn0
+// and the sweep-1 result is produced straight into those of dn1, which is what they have to become for the next step --
+// the 64 register moves per step that `dn0 = up; dn1 = o1` used to cost are gone.
+// A wall column (element 0 of the first vector of a row) stays exactly zero through its coefficients: its own value and its
+// z- and y-neighbours are walls (zero), so with By = wz = 0 for that element the update returns 0 -- no select per row.
+template <int WXT, int S, bool HAS_RHS, bool NORM, bool PRO, bool ISO>
+__device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, const ZCoef<double>& k1, const ZCoef<double>& k2, Patch<double>& dn0,
+                                         const Patch<double>& c0, Patch<double>& dn1, const Patch<double>& c1, uint32_t a_new, uint32_t a_cen,
+                                         uint32_t a_exw, uint32_t a_exr, int m1, int m2, double& pa)
+{
+    using T = double;
+    constexpr int ZR = ZV<T>::R;
+    constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * 8u;
+    const double By1a = z.cw0 ? 0.0 : k1.By, wz1a = z.cw0 ? 0.0 : k1.wz;
+    const double By2a = z.cw0 ? 0.0 : k2.By, wz2a = z.cw0 ? 0.0 : k2.wz;
+    const uint32_t a_cen1 = a_cen + z.eo1, a_cen2 = a_cen + z.eo2, a_exr1 = a_exr + z.eo1, a_exr2 = a_exr + z.eo2;
+    struct Nb {
+        T q1, q2, q3, q4;        // x-neighbours as loaded: (w, e) or, on the lanes with z.swp, (e, w); stage 1 | stage 2
+        ZVec<T> f1, f2;
+    };
+    auto load_nb = [&](int r, Nb& q) {
+        const long long grow = (long long)r * p.sx;
+        q.q1 = lds_one<T>(a_cen1 + r * rowb);
+        q.q2 = lds_one<T>(a_cen2 + r * rowb);
+        if (HAS_RHS) q.f1 = zld(z.f1 + grow);
+        if (S == 2) {
+            q.q3 = lds_one<T>(a_exr1 + r * rowb);
+            q.q4 = lds_one<T>(a_exr2 + r * rowb);
+            if (HAS_RHS) q.f2 = zld(z.f1 - p.sp + grow);
+        }
+    };
+    // the bracket of one row of one stage
+    auto bracket = [&](const ZCoef<T>& k, double Bya, double wza, const ZVec<T>& c, T w, T e, const ZVec<T>& n, const ZVec<T>& s2,
+                       const ZVec<T>& dn, const ZVec<T>& f) {
+        ZVec<T> a;
+        const double h0 = ISO ? (c.v[1] + w) + (n.v[0] + s2.v[0]) : fma(p.rho, c.v[1] + w, n.v[0] + s2.v[0]);
+        const double h1 = ISO ? (e + c.v[0]) + (n.v[1] + s2.v[1]) : fma(p.rho, e + c.v[0], n.v[1] + s2.v[1]);
+        a.v[0] = fma(k.Bz, dn.v[0], k.A * c.v[0]);
+        a.v[1] = fma(k.Bz, dn.v[1], k.A * c.v[1]);
+        a.v[0] = fma(Bya, h0, a.v[0]);
+        a.v[1] = fma(k.By, h1, a.v[1]);
+        if (HAS_RHS) {
+            a.v[0] = fma(wza, f.v[0], a.v[0]);
+            a.v[1] = fma(k.wz, f.v[1], a.v[1]);
+        }
+        return a;
+    };
+    const ZVec<T> lo1 = lds_vec<T>(a_cen - rowb), hi1 = lds_vec<T>(a_cen + ZR * rowb);     // rows -1 and ZR of the centre planes
+    ZVec<T> lo2, hi2;
+    if (S == 2) { lo2 = lds_vec<T>(a_exr - rowb); hi2 = lds_vec<T>(a_exr + ZR * rowb); }
+    Nb nb[2];
+    ZVec<T> acc1[2], acc2[2];
+    // prolongation-fused variant: the two coarse planes of this step summed, per coarse row under the patch (loaded as needed);
+    // planes without a correction (k = 0, nz-1, the idle step) run the same code with the weights 0 on whatever finite
+    // numbers the coarse ring holds (it is zero-filled at the start of the kernel)
+    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * 8u;
+    T cz[ZR / 2 + 1][2];
+    const T cs1 = (PRO && z.corr) ? 0.125 : 0.0, cs2 = (PRO && z.corr) ? 0.25 : 0.0;
+    const uint32_t cb0 = z.c0a + z.ce_own, cb1 = z.c1a + z.ce_own;
+    auto czrow = [&](int q) {
+        cz[q][0] = lds_one<T>(cb0 + q * crowb) + lds_one<T>(cb1 + q * crowb);
+        cz[q][1] = lds_one<T>(cb0 + q * crowb + 8) + lds_one<T>(cb1 + q * crowb + 8);
+    };
+    auto pre = [&](int r) {     // brackets of row r; afterwards dn0.r[r] and dn1.r[r] are dead and take their new contents
+        const Nb& q = nb[r & 1];
+        const T w1 = z.swp ? q.q2 : q.q1, e1 = z.swp ? q.q1 : q.q2;
+        acc1[r & 1] = bracket(k1, By1a, wz1a, c0.r[r], w1, e1, r == ZR - 1 ? hi1 : c0.r[r + 1 < ZR ? r + 1 : r], r == 0 ? lo1 : c0.r[r > 0 ? r - 1 : 0],
+                              dn0.r[r], q.f1);
+        dn0.r[r] = lds_vec<T>(a_new + r * rowb);      // plane t: `up` now, the centre plane of the next step
+        if (PRO) {
+            // prolongation folded in (a6): plane t takes u += P e_c as it is read, and goes back corrected to its ring slot,
+            // where the neighbours read it in the next step.  jt is odd: patch row r lies between the coarse rows (r+1)>>1
+            // and (r+2)>>1 of the tile's coarse rows (coincident when they are equal).  A wall column needs no test: the
+            // coarse wall value it would take is zero.
+            const int q0 = (1 + r) >> 1, q1 = (2 + r) >> 1;
+            if (r == 0) { czrow(0); czrow(1); }
+            else if (q1 != q0) czrow(q1);
+            const T e0 = cz[q0][0] + cz[q1][0], e1 = cz[q0][1] + cz[q1][1];
+            dn0.r[r].v[0] = fma(cs2, e0, dn0.r[r].v[0]);
+            dn0.r[r].v[1] = fma(cs1, e0 + e1, dn0.r[r].v[1]);
+            sts_vec(a_new + r * rowb, dn0.r[r]);
+        }
+        if (S == 2) {
+            const T w2 = z.swp ? q.q4 : q.q3, e2 = z.swp ? q.q3 : q.q4;
+            acc2[r & 1] = bracket(k2, By2a, wz2a, c1.r[r], w2, e2, r == ZR - 1 ? hi2 : c1.r[r + 1 < ZR ? r + 1 : r],
+                                  r == 0 ? lo2 : c1.r[r > 0 ? r - 1 : 0], dn1.r[r], q.f2);
+        }
+    };
+    load_nb(0, nb[0]);
+    if (ZR > 1) load_nb(1, nb[1]);
+    pre(0);
+#pragma unroll
+    for (int r = 0; r < ZR; ++r) {
+        const long long grow = (long long)r * p.sx;
+        if (r + 1 < ZR) pre(r + 1);
+        if (r + 2 < ZR) load_nb(r + 2, nb[r & 1]);
+        // ---------------- stage 1: sweep-1 values of row r of plane t-1 ----------------
+        ZVec<T> o1;
+        o1.v[0] = fma(k1.Bz, dn0.r[r].v[0], acc1[r & 1].v[0]);
+        o1.v[1] = fma(k1.Bz, dn0.r[r].v[1], acc1[r & 1].v[1]);
+        if (r == ZR - 1 && z.wrow) o1.v[0] = o1.v[1] = 0.0;    // the wall row j = sy, when the tile holds it as a patch row
+        if (NORM) norm_acc(pa, o1.v[0] - c0.r[r].v[0], o1.v[1] - c0.r[r].v[1], m1 & (1 << r));
+        if (S == 1) {
+            if (m1 & (1 << r)) zst(z.o_last + grow, o1);
+        } else {
+            sts_vec(a_exw + r * rowb, o1);
+            // ---------------- stage 2: sweep-2 values of row r of plane t-2 ----------------
+            ZVec<T> o2;
+            o2.v[0] = fma(k2.Bz, o1.v[0], acc2[r & 1].v[0]);
+            o2.v[1] = fma(k2.Bz, o1.v[1], acc2[r & 1].v[1]);
+            if (m2 & (1 << r)) zst(z.o_last + grow, o2);
+            dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
+        }
+    }
+}
+
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (steps come in pairs).
@@ -493,7 +633,8 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     const uint32_t a_exw = z.ex_own + (uint32_t)(t & 1) * planeb;                      // sweep-1 plane t-1 (written now)
     const uint32_t a_exr = z.ex_own + (uint32_t)((t & 1) ^ 1) * planeb;                // sweep-1 plane t-2 (written a step ago)
     if (fresh) mbar_wait32(z.bars + 8 * ring_slot<NIN>(pos), ring_par<NIN>(pos));
-    if (PRO && fresh) z_prolong<T, WXT, NIN>(p, z, t, ring_slot<NIN>(pos));
+    if (PRO) z.corr = false;
+    if (PRO && fresh) z_prolong<T, WXT, NIN, sizeof(T) == 4>(p, z, t, ring_slot<NIN>(pos));   // fp64: own rows inside the row loop
     ZCoef<T> k1, k2;
     zc_load(k1, z.coef, HAS_RHS, NORM);
     if (S == 2) zc_load(k2, z.coef - ZV<T>::NCO * ES, HAS_RHS, false);
@@ -532,6 +673,9 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             if (HAS_RHS) q.f2 = zld(z.f1 - p.sp + grow);
         }
     };
+    if constexpr (sizeof(T) == 8 && !ZERO) {
+        z_rows64<WXT, S, HAS_RHS, NORM, PRO, ISO>(p, z, k1, k2, dn0, c0, dn1, c1, a_new, a_cen, a_exw, a_exr, m1, m2, pa);
+    } else {
     RowIn rin[2];
     load_row(0, rin[0]);
 #pragma unroll
@@ -543,7 +687,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
         ZVec<T> o1;
         if (ZERO) {
 #pragma unroll
-            for (int e = 0; e < V; ++e) o1.v[e] = k1.wz * in.f1.v[e];
+            for (int e = 0; e < V; ++e) o1.v[e] = (r == ZR - 1 && z.wrow) ? T(0) : k1.wz * in.f1.v[e];
             if (z.cw0) o1.v[0] = T(0);
         } else {
             const ZVec<T> nn = r == ZR - 1 ? in.edge1 : c0.r[r + 1 < ZR ? r + 1 : r];
@@ -552,6 +696,10 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             const T w1 = z.swp ? in.e : in.w, e1 = z.swp ? in.w : in.e;
             jac_row<HAS_RHS, ISO>(k1, p.rho, p.cz, p.a2, c0.r[r], w1, e1, nn, ss, in.up0, dn0.r[r], in.f1, o1, z.cw0, rs);
             if (z.cw0) o1.v[0] = c0.r[r].v[0];
+            if (r == ZR - 1 && z.wrow) {
+#pragma unroll
+                for (int e = 0; e < V; ++e) o1.v[e] = T(0);
+            }
             if (NORM && (m1 & (1 << r))) {
                 if (sizeof(T) == 8) {
 #pragma unroll
@@ -580,6 +728,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
             if (m2 & (1 << r)) zst(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
         }
+    }
     }
     if (NORM) {
         if (sizeof(T) == 8) z.acc = fma(zc_iw2(k1), pa, z.acc);   // pa == 0 unless plane t-1 is an output plane
@@ -626,6 +775,10 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
         for (int q = threadIdx.x; q < 2 * INP; q += blockDim.x) EX[q] = T(0);
     }
     if (threadIdx.x < NCO) coef[-NCO + (int)threadIdx.x] = T(0);
+    if (PRO) {   // (planes without a correction read the coarse ring with zero weights: finite numbers, please)
+        for (int q = threadIdx.x; q < ZNCE * ZG<T, WXT>::CINP; q += blockDim.x) CE[q] = T(0);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes before the bulk copies into the same memory
+    }
     __syncthreads();
 
     const int cx0 = (wx * 32 + lane) * V;                   // first column of this thread's vector inside the tile
@@ -640,9 +793,10 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     z.in_base = smem_u32(IN);
     z.ce_base = PRO ? smem_u32(CE) : 0u;
     z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0;
+    z.c0a = z.c1a = z.ce_base; z.corr = false; z.wrow = false;
     int ring = 0;                                           // planes requested so far by this CTA (ring position)
     int cring = 0;                                          // coarse planes requested so far (PRO)
-    const long long q0 = p.items * blockIdx.x / gridDim.x, q1 = p.items * (blockIdx.x + 1) / gridDim.x;
+    const long long q0 = p.qb[blockIdx.x], q1 = p.qb[blockIdx.x + 1];
 
     for (long long q = q0; q < q1;) {
         const int tile = (int)(q / p.NP);
@@ -653,7 +807,8 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
         const int ct = p.ntx == 1 ? 0 : tx * p.COUT - V;              // first column of the tile
         // Tiles along y: patch rows [jt, jt+NR) are interior rows; the wall rows j = 0 / j = sy are only ever
         // read -- from the input halo row in sweep 1, from the (zero) guard row of the exchange plane in sweep 2.
-        const int jt = min(1 + ty * p.STEP, p.sy - NR);                // first patch row
+        // (always odd; the last tile is pulled back so that its last patch row is the wall row j = sy, which it holds at zero)
+        const int jt = min(1 + ty * p.STEP, p.sy - NR + 1);            // first patch row
         const int jlo = ty == 0 ? 1 : 1 + ty * p.STEP + H;             // rows [jlo, jhi) are this tile's output
         const int jhi = ty == p.nty - 1 ? p.sy : 1 + ty * p.STEP + NR - H;
         const int kstart = max(kb - S, 0);
@@ -705,6 +860,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
         const int jrow0 = jt + wy * ZR;                                 // grid row of patch row 0
         const int icol0 = ct + cx0;                                     // grid column of vector element 0
         z.cw0 = (icol0 == 0) || (icol0 == p.sx);
+        z.wrow = jrow0 + ZR - 1 == p.sy;
         const bool col_out = p.ntx == 1 ? true : (cx0 >= V && cx0 < TC - V && icol0 < p.sx);
         z.omask = 0;
 #pragma unroll
@@ -761,10 +917,67 @@ struct ZCfg {
     bool ok = false;
     int WX = 0, WY = 0, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
     size_t smem = 0;
+    int qb[ZQB];
 };
 
+// Work partition.  The work is the linearised list of (tile, plane) items, plane fastest; a CTA gets a contiguous range
+// and runs one z-segment per tile it touches.  A segment of n output planes costs n + W plane steps (W: the S warm-up and
+// S drain planes of the pipeline, the first step, the coefficient table and the first wait for the input ring), so equal
+// ITEM counts are not equal work: a range that straddles a tile boundary pays W twice (measured at 257^3, 148 CTAs: the
+// slowest SM was busy 113 k cycles against 98 k on average, and the 17 straddlers were the slow ones).  The ranges are
+// cut greedily for the smallest maximum COST instead: returns the largest range length.
+static int zpartition(int ntiles, int NP, int W, int ctas, int* qb)
+{
+    const long long N = (long long)ntiles * NP;
+    auto cut = [&](long long T, int* out) -> int {     // CTAs needed when none may cost more than T
+        long long q = 0;
+        int n = 0;
+        while (q < N) {
+            if (out && n <= ctas) out[n] = (int)q;
+            long long budget = T;
+            while (budget > W && q < N) {                // a segment: W + at least one plane
+                const long long tile_end = (q / NP + 1) * NP;
+                const long long take = std::min(budget - W, tile_end - q);
+                q += take;
+                budget -= take + W;
+            }
+            if (++n > ctas && !out) return n;
+        }
+        if (out)
+            for (int i = n; i <= ctas; ++i) out[i] = (int)N;
+        return n;
+    };
+    long long lo = W + 1, hi = N + (long long)W * ntiles;   // cut(hi) == 1
+    while (lo < hi) {
+        const long long mid = (lo + hi) / 2;
+        if (cut(mid, nullptr) <= ctas) hi = mid; else lo = mid + 1;
+    }
+    cut(lo, qb);
+    int longest = 0;
+    for (int i = 0; i < ctas; ++i) longest = std::max(longest, qb[i + 1] - qb[i]);
+    return longest;
+}
+
 template <typename T>
-static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro = false)
+static ZCfg zcfg_make(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro);
+
+// The launch shape is a function of the level's extents, the element type, S, the variant and the SM count: computed once
+// per process and kept (the partition is a small search, and zcfg is asked several times per cycle).
+template <typename T>
+static const ZCfg& zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro = false)
+{
+    using Key = std::tuple<int, int, int, int, int, int, int, int, int>;
+    static std::map<Key, ZCfg> cache;
+    static std::mutex mu;
+    const Key key(lv.dim, lv.nx, lv.ny, lv.nz, (int)sizeof(T), S, (int)zero + 2 * (int)pro, c->num_sms, (int)lv.coarsest);
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = cache.find(key);
+    if (it == cache.end()) it = cache.emplace(key, zcfg_make<T>(c, lv, S, zero, pro)).first;
+    return it->second;
+}
+
+template <typename T>
+static ZCfg zcfg_make(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro)
 {
     constexpr int V = ZV<T>::N;
     constexpr int NCO = ZV<T>::NCO;
@@ -794,9 +1007,11 @@ static ZCfg zcfg(const mhs_ctx* c, const Level& lv, int S, bool zero, bool pro =
     z.STEP = NR - 2 * (S - 1);
     z.nty = lv.sy - NR - 1 <= 0 ? 1 : (lv.sy - NR - 1 + z.STEP - 1) / z.STEP + 1;
     const long long items = (long long)z.ntx * z.nty * (lv.nz - 2);
+    if (items >= (1ll << 31)) return z;
     // one CTA per SM; a z-segment should be long against its S warm-up planes
-    z.ctas = (int)std::max<long long>(1, std::min<long long>(c->num_sms, items / 12));
-    z.zcap = (int)std::min<long long>(lv.nz + 1, (items + z.ctas - 1) / z.ctas + 2 * S + 3);
+    z.ctas = (int)std::max<long long>(1, std::min<long long>(std::min(c->num_sms, ZQB - 1), items / 12));
+    const int longest = zpartition(z.ntx * z.nty, lv.nz - 2, 2 * S + 2, z.ctas, z.qb);
+    z.zcap = (int)std::min<long long>(lv.nz + 1, (long long)longest + 2 * S + 3);
     z.coef_bytes = (int)(((size_t)(z.zcap + 1) * NCO * sizeof(T) + 127) / 128 * 128);
     z.in_plane = (NR + 2) * z.TC;
     const size_t plane = (size_t)z.in_plane * sizeof(T);
@@ -841,6 +1056,7 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
     p.ec = (const T*)ec; p.csp = csp;
+    for (int i = 0; i <= z.ctas; ++i) p.qb[i] = z.qb[i];
     if (z.ntx > 1) c->prof.xtiled_zsweep += 1;
     launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZV<T>::WY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (c->debug) {
@@ -882,13 +1098,13 @@ bool launch_zsweep_prolong(mhs_ctx* c, const Level& lv, const void* u, const voi
 {
     if (co.sx * 2 != lv.sx) return false;
     if (c->es == 8) {
-        const ZCfg z = zcfg<double>(c, lv, S, false, true);
+        const ZCfg& z = zcfg<double>(c, lv, S, false, true);
         if (!z.ok) return false;
         count_launch(c);
         if (rhs) { if (S == 2) zsweep_launch_pro<double, 2, true>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<double, 1, true>(c, lv, z, u, rhs, out, done, ec, co.sp); }
         else { if (S == 2) zsweep_launch_pro<double, 2, false>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<double, 1, false>(c, lv, z, u, rhs, out, done, ec, co.sp); }
     } else {
-        const ZCfg z = zcfg<float>(c, lv, S, false, true);
+        const ZCfg& z = zcfg<float>(c, lv, S, false, true);
         if (!z.ok) return false;
         count_launch(c);
         if (rhs) { if (S == 2) zsweep_launch_pro<float, 2, true>(c, lv, z, u, rhs, out, done, ec, co.sp); else zsweep_launch_pro<float, 1, true>(c, lv, z, u, rhs, out, done, ec, co.sp); }
@@ -909,7 +1125,7 @@ int launch_zsweep(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, v
     count_launch(c);
 #define ZS(T, SS, RHS, ZERO, NORM)                                                        \
     do {                                                                                  \
-        const ZCfg z = zcfg<T>(c, lv, SS, ZERO);                                          \
+        const ZCfg& z = zcfg<T>(c, lv, SS, ZERO);                                         \
         const int n = zsweep_launch<T, SS, RHS, ZERO, NORM>(c, lv, z, u, rhs, out, done); \
         return NORM ? n : 0;                                                              \
     } while (0)
