@@ -182,6 +182,9 @@ void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, con
 void launch_resid_restrict_z(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
 // the same for a big level, in separable form (no plane of u kept, the residual never formed)
 void launch_resid_restrict_sep(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
+// the same for a level WITHOUT a right-hand side (the finest 3D level), fed by the bulk-copy engine (mhs_kernels_restrict.cu);
+// down: walk down in z.  false: shape not supported, nothing launched.
+bool launch_resid_restrict_ring(mhs_ctx* c, const Level& fine, const void* u, const Level& coarse, void* rhs_c, int down, const int* done);
 void launch_prolong_v(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, int reverse, const int* done);
 // ---- temporally blocked smoother (mhs_kernels_zfused.cu) ----
 bool zsweep_ok(const mhs_ctx* c, const Level& lv);

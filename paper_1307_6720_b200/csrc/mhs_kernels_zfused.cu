@@ -481,10 +481,10 @@ __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* til
 }
 
 // pa += d0^2 + d1^2 where `on` is set: predicated FMAs (written as a select ptxas makes 2 FSEL per value of them)
-__device__ __forceinline__ void norm_acc(double& pa, double d0, double d1, int on)
+__device__ __forceinline__ void norm_acc(double& pa, double& pb, double d0, double d1, int on)
 {
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p fma.rn.f64 %0, %1, %1, %0;\n\t@p fma.rn.f64 %0, %2, %2, %0;\n\t}"
-        : "+d"(pa)
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %4, 0;\n\t@p fma.rn.f64 %0, %2, %2, %0;\n\t@p fma.rn.f64 %1, %3, %3, %1;\n\t}"
+        : "+d"(pa), "+d"(pb)
         : "d"(d0), "d"(d1), "r"(on));
 }
 
@@ -581,6 +581,7 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
                                   r == 0 ? lo2 : c1.r[r > 0 ? r - 1 : 0], dn1.r[r], q.f2);
         }
     };
+    double pn[4] = {0.0, 0.0, 0.0, 0.0};     // four partial sums of the norm: dependency chains of 4 FMAs instead of 16
     load_nb(0, nb[0]);
     if (ZR > 1) load_nb(1, nb[1]);
     pre(0);
@@ -594,7 +595,7 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
         o1.v[0] = fma(k1.Bz, dn0.r[r].v[0], acc1[r & 1].v[0]);
         o1.v[1] = fma(k1.Bz, dn0.r[r].v[1], acc1[r & 1].v[1]);
         if (r == ZR - 1 && z.wrow) o1.v[0] = o1.v[1] = 0.0;    // the wall row j = sy, when the tile holds it as a patch row
-        if (NORM) norm_acc(pa, o1.v[0] - c0.r[r].v[0], o1.v[1] - c0.r[r].v[1], m1 & (1 << r));
+        if (NORM) norm_acc(pn[(2 * r) & 3], pn[(2 * r + 1) & 3], o1.v[0] - c0.r[r].v[0], o1.v[1] - c0.r[r].v[1], m1 & (1 << r));
         if (S == 1) {
             if (m1 & (1 << r)) zst(z.o_last + grow, o1);
         } else {
@@ -607,6 +608,7 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
         }
     }
+    if (NORM) pa = (pn[0] + pn[1]) + (pn[2] + pn[3]);
 }
 
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring

@@ -55,7 +55,7 @@ WORKLOADS = {
 # fast: the default launch shapes;  big: the big-level (HBM-bound) kernels forced onto these small grids;
 # unfused: tuned kernels without temporal blocking / separable restriction;  reference: the paper's kernel design
 # big_sep: as big, with the prolongation kept a pass of its own (by default it is folded into the first post-smoothing pass)
-VARIANTS = {"fast": 0, "big": 8, "big_sep": 8 | 16, "unfused": 4 | 8, "reference": 1}
+VARIANTS = {"fast": 0, "big": 8, "big_sep": 8 | 16, "big_loaded": 8 | 64, "unfused": 4 | 8, "reference": 1}
 
 
 def flags_of(B, variant):
@@ -113,6 +113,9 @@ def test_operators_3d(B, orc, name, dtype, variant):
             S.op_vcycle(3, lvl)
             uv = orc.vcycle3(u_in, rhs, cl, w.alpha, Ll, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post)
             assert relmax(host(S.level_get(3, lvl, 0)), uv) <= 20 * OPTOL[dtype]
+        # the finest level's residual + restriction: bulk-copy fed kernel on the big-level path, the loading one on request
+        ring = S.profile()["ring_restrict"]
+        assert (ring >= 2) if variant in ("big", "big_sep") else (ring == 0) if variant != "fast" else True
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
