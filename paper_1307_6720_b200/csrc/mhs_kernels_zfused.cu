@@ -549,31 +549,36 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
     // planes without a correction (k = 0, nz-1, the idle step) run the same code with the weights 0 on whatever finite
     // numbers the coarse ring holds (it is zero-filled at the start of the kernel)
     constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * 8u;
-    T cz[ZR / 2 + 1][2];
+    T cz[ZR / 2 + 1][2], czr[ZR / 2 + 1][4];
+    ZVec<T> upb[2];           // plane t of the rows r, r+1 as loaded (uncorrected), two rows ahead of their correction
     const T cs1 = (PRO && z.corr) ? 0.125 : 0.0, cs2 = (PRO && z.corr) ? 0.25 : 0.0;
     const uint32_t cb0 = z.c0a + z.ce_own, cb1 = z.c1a + z.ce_own;
-    auto czrow = [&](int q) {
-        cz[q][0] = lds_one<T>(cb0 + q * crowb) + lds_one<T>(cb1 + q * crowb);
-        cz[q][1] = lds_one<T>(cb0 + q * crowb + 8) + lds_one<T>(cb1 + q * crowb + 8);
+    auto czload = [&](int q) {    // (issued well ahead of czsum: a store to shared memory sits between every two rows, and no
+                                  //  load can be moved up across it by the assembler)
+        czr[q][0] = lds_one<T>(cb0 + q * crowb); czr[q][1] = lds_one<T>(cb1 + q * crowb);
+        czr[q][2] = lds_one<T>(cb0 + q * crowb + 8); czr[q][3] = lds_one<T>(cb1 + q * crowb + 8);
     };
+    auto czsum = [&](int q) { cz[q][0] = czr[q][0] + czr[q][1]; cz[q][1] = czr[q][2] + czr[q][3]; };
     auto pre = [&](int r) {     // brackets of row r; afterwards dn0.r[r] and dn1.r[r] are dead and take their new contents
         const Nb& q = nb[r & 1];
         const T w1 = z.swp ? q.q2 : q.q1, e1 = z.swp ? q.q1 : q.q2;
         acc1[r & 1] = bracket(k1, By1a, wz1a, c0.r[r], w1, e1, r == ZR - 1 ? hi1 : c0.r[r + 1 < ZR ? r + 1 : r], r == 0 ? lo1 : c0.r[r > 0 ? r - 1 : 0],
                               dn0.r[r], q.f1);
-        dn0.r[r] = lds_vec<T>(a_new + r * rowb);      // plane t: `up` now, the centre plane of the next step
+        if (!PRO) dn0.r[r] = lds_vec<T>(a_new + r * rowb);      // plane t: `up` now, the centre plane of the next step
         if (PRO) {
             // prolongation folded in (a6): plane t takes u += P e_c as it is read, and goes back corrected to its ring slot,
             // where the neighbours read it in the next step.  jt is odd: patch row r lies between the coarse rows (r+1)>>1
             // and (r+2)>>1 of the tile's coarse rows (coincident when they are equal).  A wall column needs no test: the
             // coarse wall value it would take is zero.
             const int q0 = (1 + r) >> 1, q1 = (2 + r) >> 1;
-            if (r == 0) { czrow(0); czrow(1); }
-            else if (q1 != q0) czrow(q1);
+            if (r == 0) { czsum(0); czsum(1); }
+            else if (q1 != q0) czsum(q1);
             const T e0 = cz[q0][0] + cz[q1][0], e1 = cz[q0][1] + cz[q1][1];
-            dn0.r[r].v[0] = fma(cs2, e0, dn0.r[r].v[0]);
-            dn0.r[r].v[1] = fma(cs1, e0 + e1, dn0.r[r].v[1]);
+            dn0.r[r].v[0] = fma(cs2, e0, upb[r & 1].v[0]);
+            dn0.r[r].v[1] = fma(cs1, e0 + e1, upb[r & 1].v[1]);
             sts_vec(a_new + r * rowb, dn0.r[r]);
+            if (r + 2 < ZR) upb[r & 1] = lds_vec<T>(a_new + (r + 2) * rowb);
+            if (r + 2 < ZR && ((4 + r) >> 1) != ((3 + r) >> 1)) czload((4 + r) >> 1);      // the coarse row that row r+2 adds
         }
         if (S == 2) {
             const T w2 = z.swp ? q.q4 : q.q3, e2 = z.swp ? q.q3 : q.q4;
@@ -582,14 +587,19 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
         }
     };
     double pn[4] = {0.0, 0.0, 0.0, 0.0};     // four partial sums of the norm: dependency chains of 4 FMAs instead of 16
+    if (PRO) {
+        upb[0] = lds_vec<T>(a_new);
+        upb[1] = lds_vec<T>(a_new + rowb);
+        czload(0); czload(1);                  // (row r+2's new coarse row is requested while row r is corrected)
+    }
     load_nb(0, nb[0]);
     if (ZR > 1) load_nb(1, nb[1]);
     pre(0);
 #pragma unroll
     for (int r = 0; r < ZR; ++r) {
         const long long grow = (long long)r * p.sx;
+        if (r + 2 < ZR) load_nb(r + 2, nb[r & 1]);     // (ahead of pre(): its store of the corrected row would pin these loads behind it)
         if (r + 1 < ZR) pre(r + 1);
-        if (r + 2 < ZR) load_nb(r + 2, nb[r & 1]);
         // ---------------- stage 1: sweep-1 values of row r of plane t-1 ----------------
         ZVec<T> o1;
         o1.v[0] = fma(k1.Bz, dn0.r[r].v[0], acc1[r & 1].v[0]);
