@@ -534,7 +534,7 @@ mhs_status run_cycles(mhs_ctx* ctx, std::vector<Level>& Ls, double tol, int max_
             const double target = tol * h->r0;
             if (rl > 0.0 && rp > rl && target > 0.0 && rl > target) {
                 const double need = std::ceil(std::log(target / rl) / std::log(rl / rp));
-                want = (int)std::min(8.0, std::max(1.0, h->cycles + need + 1 - issued));
+                want = (int)std::min(16.0, std::max(1.0, h->cycles + need + 1 - issued));
             }
         }
         const int n = std::min(sync_each ? 1 : want, max_cycles - issued);
