@@ -82,6 +82,8 @@ typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 
 #define MHS_FLAG_NO_PDL            32 /* launch every kernel fully serialised (no programmatic dependent launch)   */
 #define MHS_FLAG_LOADED_RESTRICT   64 /* finest level: residual + restriction by the kernel that loads through the L1
                                         instead of the bulk-copy fed one; for A/B tests                         */
+#define MHS_FLAG_LOADED_FIELDS    128 /* mhs_fields by the register z-streaming kernel instead of the bulk-copy fed
+                                        one; for A/B tests                                                      */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 
@@ -153,6 +155,7 @@ typedef struct {
                                          narrower than a grid row (rows wider than 256 fp64 / 512 fp32 columns)  */
     long long ring_restrict;          /* residual + restriction launches (any level) that ran in the bulk-copy fed
                                          kernel                                                                 */
+    long long ring_fields;            /* mhs_fields calls served by the bulk-copy fed kernel                    */
 } mhs_profile;
 
 /* Fill *o with the defaults: fp64, omega 2/3, V(2,2), full coarsening, boundary_tol 1e-10,

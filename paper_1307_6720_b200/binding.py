@@ -25,6 +25,7 @@ MHS_FLAG_BIG_LEVEL_KERNELS = 8
 MHS_FLAG_SEPARATE_PROLONG = 16
 MHS_FLAG_NO_PDL = 32
 MHS_FLAG_LOADED_RESTRICT = 64
+MHS_FLAG_LOADED_FIELDS = 128
 MHS_SMOOTH_JACOBI, MHS_SMOOTH_ZLINE = 0, 1
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8
@@ -65,7 +66,7 @@ class mhs_solve_info(C.Structure):
 class mhs_profile(C.Structure):
     _fields_ = [("launches", C.c_longlong * MHS_KC_COUNT), ("ms", C.c_double * MHS_KC_COUNT),
                 ("sweeps_l0", C.c_longlong), ("fused_prolong_l0", C.c_longlong), ("xtiled_zsweep", C.c_longlong),
-                ("ring_restrict", C.c_longlong)]
+                ("ring_restrict", C.c_longlong), ("ring_fields", C.c_longlong)]
 
 
 class MHSError(RuntimeError):
@@ -250,7 +251,7 @@ def mhs_get_profile(h):
     names = [lib().mhs_kernel_class_name(k).decode() for k in range(MHS_KC_COUNT)]
     return dict(launches={n: int(p.launches[k]) for k, n in enumerate(names)},
                 ms={n: float(p.ms[k]) for k, n in enumerate(names)}, sweeps_l0=int(p.sweeps_l0),
-                fused_prolong_l0=int(p.fused_prolong_l0), xtiled_zsweep=int(p.xtiled_zsweep), ring_restrict=int(p.ring_restrict),
+                fused_prolong_l0=int(p.fused_prolong_l0), xtiled_zsweep=int(p.xtiled_zsweep), ring_restrict=int(p.ring_restrict), ring_fields=int(p.ring_fields),
                 total_launches=int(sum(p.launches)))
 
 

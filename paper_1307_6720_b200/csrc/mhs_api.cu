@@ -987,7 +987,10 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
     if (!B && !p && !rho) return MHS_OK;
     Scope sc(ctx, MHS_KC_FIELDS);
     const Level& l0 = ctx->L3[0];
-    if (!(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fields_z_ok(ctx, l0)) {
+    if (!(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_LOADED_FIELDS)) && launch_fields_ring(ctx, l0, l0.u, B, p, rho)) {
+        ctx->prof.ring_fields += 1;
+        launch_fields_ref(ctx, l0, l0.u, B, p, rho, true);
+    } else if (!(ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) && fields_z_ok(ctx, l0)) {
         launch_fields_z(ctx, l0, l0.u, B, p, rho);
         launch_fields_ref(ctx, l0, l0.u, B, p, rho, true);
     } else {

@@ -161,6 +161,8 @@ void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void
 // ---- one-pass field recovery (mhs_kernels_fields.cu): planes 1 .. nz-2 ----
 bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
+// the same, fed by the bulk-copy engine (mhs_kernels_fields_ring.cu); false: shape not supported, nothing launched
+bool launch_fields_ring(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);
 void launch_diagnostics(mhs_ctx* c, const Level& lv, const void* B, void* absB, void* J, void* absJ);
 // ---- solver variants (mhs_kernels_variants.cu): z-line Jacobi, full-multigrid start ----
 bool zline_ok(const mhs_ctx* c, const Level& lv);

@@ -55,7 +55,7 @@ WORKLOADS = {
 # fast: the default launch shapes;  big: the big-level (HBM-bound) kernels forced onto these small grids;
 # unfused: tuned kernels without temporal blocking / separable restriction;  reference: the paper's kernel design
 # big_sep: as big, with the prolongation kept a pass of its own (by default it is folded into the first post-smoothing pass)
-VARIANTS = {"fast": 0, "big": 8, "big_sep": 8 | 16, "big_loaded": 8 | 64, "unfused": 4 | 8, "reference": 1}
+VARIANTS = {"fast": 0, "big": 8, "big_sep": 8 | 16, "big_loaded": 8 | 64 | 128, "unfused": 4 | 8, "reference": 1}
 
 
 def flags_of(B, variant):
