@@ -55,7 +55,13 @@ struct __align__(2 * sizeof(T)) Pair {
     T a, b;
 };
 
-constexpr int RR_RC = 4;       // coarse rows per thread
+#ifndef MHS_RR_RC
+#define MHS_RR_RC 4
+#endif
+#ifndef MHS_RR_NT
+#define MHS_RR_NT 256
+#endif
+constexpr int RR_RC = MHS_RR_RC;       // coarse rows per thread
 constexpr int RR_MAXRING = 6;
 
 template <typename T>
@@ -206,7 +212,7 @@ bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void*
     constexpr int RC = RR_RC;
     const int ncx = f.sx / 2;
     if (f.sx % 2 || co.sx * 2 != f.sx || ncx < 8 || ncx > 512 || ((size_t)f.sx * sizeof(T)) % 16) return false;
-    int G = std::max(1, 256 / ncx);
+    int G = std::max(1, MHS_RR_NT / ncx);
     while (G > 1 && RC * G > co.sy - 1) G >>= 1;                       // no more rows than the level has
     const size_t limit = 227 * 1024 - 1024;
     int nring = 0;

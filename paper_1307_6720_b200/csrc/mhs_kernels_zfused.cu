@@ -142,6 +142,22 @@ template <typename T>
 __device__ __forceinline__ ZVec<T> zld(const T* p) { return *reinterpret_cast<const ZVec<T>*>(p); }
 template <typename T>
 __device__ __forceinline__ void zst(T* p, const ZVec<T>& a) { *reinterpret_cast<ZVec<T>*>(p) = a; }
+// MHS_ST_HINT: 1 = st.global.cs (streaming), 2 = L2::evict_first policy on the output stores of the fp64 passes
+#ifndef MHS_ST_HINT
+#define MHS_ST_HINT 0
+#endif
+__device__ __forceinline__ void zst_out(double* p, const ZVec<double>& a)
+{
+#if MHS_ST_HINT == 1
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a.v[0]), "d"(a.v[1]) : "memory");
+#elif MHS_ST_HINT == 2
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(a.v[0]), "d"(a.v[1]), "l"(pol) : "memory");
+#else
+    *reinterpret_cast<ZVec<double>*>(p) = a;
+#endif
+}
 
 // Per-plane coefficients of one sweep (warp-uniform, read from the shared table).
 //   fp64 (expanded update):  u' = A u + By (rho (e+w) + (n+s)) + Bz (up+dn) + wz f ;  iw2 = (D/omega)^2 for the norm
@@ -607,14 +623,14 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
         if (r == ZR - 1 && z.wrow) o1.v[0] = o1.v[1] = 0.0;    // the wall row j = sy, when the tile holds it as a patch row
         if (NORM) norm_acc(pn[(2 * r) & 3], pn[(2 * r + 1) & 3], o1.v[0] - c0.r[r].v[0], o1.v[1] - c0.r[r].v[1], m1 & (1 << r));
         if (S == 1) {
-            if (m1 & (1 << r)) zst(z.o_last + grow, o1);
+            if (m1 & (1 << r)) zst_out(z.o_last + grow, o1);
         } else {
             sts_vec(a_exw + r * rowb, o1);
             // ---------------- stage 2: sweep-2 values of row r of plane t-2 ----------------
             ZVec<T> o2;
             o2.v[0] = fma(k2.Bz, o1.v[0], acc2[r & 1].v[0]);
             o2.v[1] = fma(k2.Bz, o1.v[1], acc2[r & 1].v[1]);
-            if (m2 & (1 << r)) zst(z.o_last + grow, o2);
+            if (m2 & (1 << r)) zst_out(z.o_last + grow, o2);
             dn1.r[r] = o1;  // becomes the sweep-1 centre plane of the next step
         }
     }
