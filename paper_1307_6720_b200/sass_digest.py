@@ -13,7 +13,7 @@ import sys
 
 from . import build as _build
 
-DEFAULT = r"k_zsweep<double, 4, 2, false, false, (true, false|false, true)>|k_resid_restrict_sep<double|k_fields_z<double|k_zline<double, false>|k_fieldlines<double>|k_cluster<double, true>"
+DEFAULT = r"k_zsweep<double, 4, 2, false, false, (true, false|false, true), true>|k_resid_restrict_ring<double>|k_fields_ring<double, 256|k_resid_restrict_sep<double, 4, false>|k_fields_z<double|k_zline<double, false>|k_fieldlines<double>|k_cluster<double, true>"
 
 
 def demangle(names):
