@@ -13,7 +13,7 @@ import sys
 
 from . import build as _build
 
-DEFAULT = r"k_zsweep<double, 4, 2, false, false, (true, false|false, true), true>|k_resid_restrict_ring<double>|k_fields_ring<double, 256|k_resid_restrict_sep<double, 4, false>|k_fields_z<double|k_zline<double, false>|k_fieldlines<double>|k_cluster<double, true>"
+DEFAULT = r"k_zsweep<double, 4, 2, 0, 0, (1, 0|0, 1), 1>|k_resid_restrict_ring<double>|k_fields_ring<double, 256|k_resid_restrict_sep<double, 4, 0>|k_fields_z<double|k_zline<double, 0>|k_fieldlines<double>|k_cluster<double, 1>"
 
 
 def demangle(names):
@@ -54,7 +54,7 @@ def main(pattern=DEFAULT):
     print("# SASS digest of %s\n" % lib.split("/")[-1])
     print("Command: `python -m paper_1307_6720_b200.sass_digest` (cuobjdump -sass / -res-usage of the in-tree library; static counts, whole kernel).\n")
     for n in names:
-        d = dem.get(n, n)
+        d = re.sub(r"\((int|bool)\)", "", dem.get(n, n))      # cu++filt writes template arguments as (int)4, (bool)0
         if not rx.search(d):
             continue
         h = hist[n]
