@@ -743,3 +743,38 @@ def test_fields_parity_fp32_on_a_smooth_potential(B, orc, name, variant):
         ep = relmax(host(pg), ref[3])
         er = np.abs(host(rg) - ref[4]).max() / np.abs(ref[4]).max()
         assert eB <= 2e-5 and ep <= 2e-5 and er <= 2e-4, (eB, ep, er)
+
+
+@pytest.mark.parametrize("nx,dtype", [(513, torch.float64), (1025, torch.float32), (257, torch.float64), (129, torch.float32)])
+def test_fields_ring_row_pitches(B, orc, nx, dtype):
+    """The bulk-copy fed field kernel at every row pitch it is compiled for that the other tests do not reach at oracle size
+    (pitch 512 fp64 and 1024 fp32 are what configs[3] and configs[4] run on; one thread group per column there): a smooth
+    potential with zero side and top walls on an nx x 65 x 33 slab, every node of B, p, rho against the oracle."""
+    w = inputs.small(nx=nx, ny=65, nz=33, L=(4.0, 1.0, 0.5), seed=21)
+    z = np.linspace(0.0, w.Lz, w.nz)[:, None, None]
+    y = np.linspace(0.0, w.Ly, w.ny)[None, :, None]
+    x = np.linspace(0.0, w.Lx, w.nx)[None, None, :]
+    P = np.sin(np.pi * x / w.Lx) * np.sin(2 * np.pi * y / w.Ly) * (1.0 - z / w.Lz) * np.exp(-3.0 * z) * (1.0 + 0.3 * np.cos(5 * x))
+    P[:, 0, :] = P[:, -1, :] = 0.0; P[:, :, 0] = P[:, :, -1] = 0.0; P[-1] = 0.0
+    with B.Solver.from_workload(w, dtype=dtype) as S:
+        S.set_potential(dev(P, dtype))
+        Pg = host(S.get_potential())
+        Bg, pg, rg = S.fields()
+        assert S.profile()["ring_fields"] == 1
+        ref = orc.fields(Pg, w.f, w.alpha, w.L, w.p_b, w.rho_b, mu0=w.mu0, g=w.g)
+        scaleB = max(np.abs(r).max() for r in ref[:3])
+        eB = max(np.abs(host(Bg)[q] - ref[q]).max() for q in range(3)) / scaleB
+        ep = relmax(host(pg), ref[3])
+        er = np.abs(host(rg) - ref[4]).max() / np.abs(ref[4]).max()
+        # (fp32: second differences at h = 1/256 amplify the rounding of P by 1/h^2; the bound is that arithmetic's, the
+        #  kernel that loads through the L1 must agree with the bulk-copy fed one far inside it)
+        tb, tr = (1e-12, 1e-10) if dtype == torch.float64 else (3e-4, 5e-3)
+        assert eB <= tb and ep <= tb and er <= tr, (eB, ep, er)
+    with B.Solver.from_workload(w, dtype=dtype, flags=B.MHS_FLAG_LOADED_FIELDS) as S2:
+        S2.set_potential(dev(P, dtype))
+        B2, p2, r2 = S2.fields()
+        assert S2.profile()["ring_fields"] == 0
+        tol = 1e-13 if dtype == torch.float64 else 2e-6
+        assert (Bg - B2).abs().max().item() <= tol * scaleB
+        assert (pg - p2).abs().max().item() <= tol * float(np.abs(ref[3]).max())
+        assert (rg - r2).abs().max().item() <= 10 * tol * float(np.abs(ref[4]).max())
