@@ -307,16 +307,24 @@ struct ZCtx {
     int czoff, cnext;             // ring position of coarse plane K is czoff + K; next coarse plane to request
     int jt, Jb;                   // first patch row of the tile (always odd); first coarse row held in a coarse slot
     uint32_t c0a, c1a;            // this step's two coarse planes (shared-space addresses), set by z_prolong
+    // ring positions kept incrementally (a ring of 3 would otherwise cost a division per use and step):
+    int rs;                       // ring slot of plane t (== (zoff + t) % NIN), rp: its mbarrier parity
+    uint32_t rp;
+    int cs0;                      // prolongation-fused variant: coarse slot of coarse plane t >> 1, cp0: its parity
+    uint32_t cp0;
+    // the halo vector this thread corrects (prolongation-fused variant), fixed per segment
+    bool h_ok;                    //   it exists and lies on an interior row
+    uint32_t h_a, h_co, h_dj;     //   byte offsets: inside a ring slot, inside a coarse slot, to the second coarse row
+    bool h_c0;                    //   its element 0 is a wall column
     bool corr;                    // the plane that arrives in this step takes a correction (interior plane)
     bool wrow;                    // the last patch row of this thread is the wall row j = sy (last tile along y): held at zero
 };
 
 // warp 0: request input plane `k` of the tile into ring slot nload % NIN
 template <typename T, int WXT, int NIN>
-__device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int nload, int k)
+__device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint32_t bars, T* IN, int slot, int k)
 {
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
-    const int slot = ring_slot<NIN>(nload);
     constexpr int TCc = ZG<T, WXT>::TC, INP = ZG<T, WXT>::INP;
     T* dst = IN + (size_t)slot * INP;
     const T* src = tile_src + p.sp * k;
@@ -344,6 +352,7 @@ template <typename T, int WXT, int NIN>
 __device__ __forceinline__ void c_request(const ZP<T>& p, ZCtx<T>& z, int kfine)
 {
     constexpr int CINP = ZG<T, WXT>::CINP, CSX = ZG<T, WXT>::CSX;
+    if (threadIdx.x >= 32) return;      // (cnext lives in warp 0)
     const int klast = min(min(kfine, z.kend_in), p.nz - 2);
     if (klast < 1) return;
     const int kneed = (klast + 1) >> 1;
@@ -391,11 +400,16 @@ __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* t
     if (!ZERO && may_issue) {
         const int k = z.t + NIN - 1;      // the slot of plane t-1 is free: request plane t+NIN-1 into it
         if (k <= z.kend_in) {
-            if (threadIdx.x < 32) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, z.zoff + k, k);
+            // (zoff + k) % NIN is the slot of plane t-1
+            if (threadIdx.x < 32) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, z.rs == 0 ? NIN - 1 : z.rs - 1, k);
             if (PRO) c_request<T, WXT, NIN>(p, z, k + 1);   // (one plane ahead: the coarse plane is there when its fine plane lands)
         }
     }
     ++z.t;
+    if (++z.rs == NIN) { z.rs = 0; z.rp ^= 1u; }
+    if (PRO && !(z.t & 1)) {            // t became even: t >> 1 moved on
+        if (++z.cs0 == ZNCE) { z.cs0 = 0; z.cp0 ^= 1u; }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -448,22 +462,24 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int
     z.corr = false;
     if (t < 1 || t > p.nz - 2) return;
     z.corr = true;
-    const int K0 = t >> 1, K1 = (t + 1) >> 1;
-    const int p0 = z.czoff + K0, p1 = z.czoff + K1;
-    mbar_wait32(z.bars + 8 * (NIN + p0 % ZNCE), (uint32_t)((p0 / ZNCE) & 1));
-    mbar_wait32(z.bars + 8 * (NIN + p1 % ZNCE), (uint32_t)((p1 / ZNCE) & 1));
-    const uint32_t c0a = z.ce_base + (uint32_t)(p0 % ZNCE) * cplaneb, c1a = z.ce_base + (uint32_t)(p1 % ZNCE) * cplaneb;
+    // coarse planes t >> 1 (slot cs0) and (t + 1) >> 1 (the next slot when t is odd)
+    const int s0 = z.cs0;
+    int s1 = s0;
+    uint32_t q1 = z.cp0;
+    if (t & 1) {
+        if (++s1 == ZNCE) { s1 = 0; q1 ^= 1u; }
+    }
+    mbar_wait32(z.bars + 8 * (NIN + s0), z.cp0);
+    mbar_wait32(z.bars + 8 * (NIN + s1), q1);
+    const uint32_t c0a = z.ce_base + (uint32_t)s0 * cplaneb, c1a = z.ce_base + (uint32_t)s1 * cplaneb;
     const uint32_t a_pl = z.in_own + (uint32_t)slot * planeb;
     z.c0a = c0a; z.c1a = c1a;
     if (ROWS) z_prolong_rows<T, WXT, 1>(z, a_pl, c0a, c1a);     // (jt is odd and patch rows start ZR-aligned from it)
-    // the halo rows of the tile (fine rows jt-1 and jt+NR): one vector per thread
-    const int nvr = TC / V;
-    const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
-    const int jh = which ? z.jt + NR : z.jt - 1;
-    if (which < 2 && jh >= 1 && jh < p.sy) {
-        const uint32_t a = z.in_base + (uint32_t)slot * planeb + (uint32_t)(((which ? NR + 1 : 0) * TC + hv * V) * ES);
-        const uint32_t co = (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)ES);
-        const uint32_t dj = (jh & 1) ? crowb : 0u;      // J1 = J0 + (j odd)
+    // the halo rows of the tile (fine rows jt-1 and jt+NR): one vector per thread (which one: fixed per segment, z.h_*)
+    if (z.h_ok) {
+        const uint32_t a = z.in_base + (uint32_t)slot * planeb + z.h_a;
+        const uint32_t co = z.h_co, dj = z.h_dj;
+        const bool hv_in = !z.h_c0;
         ZVec<T> v = lds_vec<T>(a);
         T c[VC + 1];
 #pragma unroll
@@ -473,10 +489,11 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int
 #pragma unroll
         for (int e = 0; e < V; ++e) {
             const T sum = (e & 1) ? (c[e >> 1] + c[(e >> 1) + 1]) : T(2) * c[e >> 1];
-            if (e > 0 || hv > 0) v.v[e] += T(0.125) * sum;
+            if (e > 0 || hv_in) v.v[e] += T(0.125) * sum;
         }
         sts_vec(a, v);
     }
+    (void)TC; (void)NR; (void)crowb; (void)VC;
 }
 
 // First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
@@ -486,10 +503,9 @@ __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* til
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int NIN = PRO ? 3 : ZNIN;
     if (!ZERO) {
-        const int pos = z.zoff + z.t;
-        mbar_wait32(z.bars + 8 * ring_slot<NIN>(pos), ring_par<NIN>(pos));
-        if (PRO) z_prolong<T, WXT, NIN>(p, z, z.t, ring_slot<NIN>(pos));
-        const uint32_t a = z.in_own + (uint32_t)ring_slot<NIN>(pos) * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
+        mbar_wait32(z.bars + 8 * z.rs, z.rp);
+        if (PRO) z_prolong<T, WXT, NIN>(p, z, z.t, z.rs);
+        const uint32_t a = z.in_own + (uint32_t)z.rs * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
 #pragma unroll
         for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(ZG<T, WXT>::TC * sizeof(T)));
     }
@@ -653,16 +669,15 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     const bool in1 = (unsigned)(t - 1 - z.kb) < (unsigned)z.nout;   // plane t-1 is an output plane of this segment
     const bool in2 = (unsigned)(t - 2 - z.kb) < (unsigned)z.nout;
     const bool fresh = !ZERO && t <= z.kend_in;                      // a new input plane arrives in this step
-    const int pos = z.zoff + t;
     // !fresh (only the step after the top plane): the slot holds an older plane -- finite numbers that meet Bz = 0
     constexpr int NIN = PRO ? 3 : ZNIN;
-    const uint32_t a_new = z.in_own + (uint32_t)ring_slot<NIN>(pos) * planeb;          // plane t
-    const uint32_t a_cen = z.in_own + (uint32_t)ring_slot<NIN>(pos - 1) * planeb;      // plane t-1
+    const uint32_t a_new = z.in_own + (uint32_t)z.rs * planeb;                                   // plane t
+    const uint32_t a_cen = z.in_own + (uint32_t)(z.rs == 0 ? NIN - 1 : z.rs - 1) * planeb;       // plane t-1
     const uint32_t a_exw = z.ex_own + (uint32_t)(t & 1) * planeb;                      // sweep-1 plane t-1 (written now)
     const uint32_t a_exr = z.ex_own + (uint32_t)((t & 1) ^ 1) * planeb;                // sweep-1 plane t-2 (written a step ago)
-    if (fresh) mbar_wait32(z.bars + 8 * ring_slot<NIN>(pos), ring_par<NIN>(pos));
+    if (fresh) mbar_wait32(z.bars + 8 * z.rs, z.rp);
     if (PRO) z.corr = false;
-    if (PRO && fresh) z_prolong<T, WXT, NIN, sizeof(T) == 4>(p, z, t, ring_slot<NIN>(pos));   // fp64: own rows inside the row loop
+    if (PRO && fresh) z_prolong<T, WXT, NIN, sizeof(T) == 4>(p, z, t, z.rs);   // fp64: own rows inside the row loop
     ZCoef<T> k1, k2;
     zc_load(k1, z.coef, HAS_RHS, NORM);
     if (S == 2) zc_load(k2, z.coef - ZV<T>::NCO * ES, HAS_RHS, false);
@@ -822,6 +837,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     z.ce_base = PRO ? smem_u32(CE) : 0u;
     z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0;
     z.c0a = z.c1a = z.ce_base; z.corr = false; z.wrow = false;
+    z.rs = 0; z.rp = 0; z.cs0 = 0; z.cp0 = 0; z.h_ok = false; z.h_a = z.h_co = z.h_dj = 0; z.h_c0 = false;
     int ring = 0;                                           // planes requested so far by this CTA (ring position)
     int cring = 0;                                          // coarse planes requested so far (PRO)
     const long long q0 = p.qb[blockIdx.x], q1 = p.qb[blockIdx.x + 1];
@@ -865,10 +881,12 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
             coef[i] = v;
         }
         z.zoff = ring - kstart;
+        z.rs = ring_slot<NIN>(ring);
+        z.rp = ring_par<NIN>(ring);
         if (!ZERO) {
             const int n = min(NIN, kend_in - kstart + 1);
             if (warp == 0)
-                for (int i = 0; i < n; ++i) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, ring + i, kstart + i);
+                for (int i = 0; i < n; ++i) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, ring_slot<NIN>(ring + i), kstart + i);
             ring += kend_in - kstart + 1;
             if (PRO) {
                 // coarse planes (kfirst >> 1) .. ((klast + 1) >> 1) serve the corrected fine planes kfirst .. klast
@@ -878,8 +896,23 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
                 const int kfirst = max(kstart, 1), klast = min(kend_in, p.nz - 2);
                 z.cnext = kfirst >> 1;
                 z.czoff = cring - z.cnext;
+                {   // ring position of coarse plane kstart >> 1 (== kfirst >> 1)
+                    const int p0 = z.czoff + (kstart >> 1);
+                    z.cs0 = p0 % ZNCE;
+                    z.cp0 = (uint32_t)((p0 / ZNCE) & 1);
+                }
                 if (klast >= kfirst) cring += ((klast + 1) >> 1) - z.cnext + 1;
                 c_request<T, WXT, NIN>(p, z, kstart + n);
+                // the halo vector this thread corrects: row jt-1 (threads 0 .. TC/V-1) or row jt+NR (the next TC/V threads)
+                constexpr int nvr = TC / V;
+                constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * sizeof(T);
+                const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
+                const int jh = which ? jt + NR : jt - 1;
+                z.h_ok = which < 2 && jh >= 1 && jh < p.sy;
+                z.h_a = (uint32_t)(((which ? NR + 1 : 0) * TC + hv * V) * (int)sizeof(T));
+                z.h_co = (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)sizeof(T));
+                z.h_dj = (jh & 1) ? crowb : 0u;
+                z.h_c0 = hv == 0;
             }
         }
         __syncthreads();   // coefficient table visible
