@@ -62,7 +62,13 @@ struct __align__(2 * sizeof(T)) Pair {
 #define MHS_RR_NT 256
 #endif
 constexpr int RR_RC = MHS_RR_RC;       // coarse rows per thread
-constexpr int RR_MAXRING = 6;
+#ifndef MHS_RR_RINGCAP
+#define MHS_RR_RINGCAP 6
+#endif
+#ifndef MHS_RR_CPS
+#define MHS_RR_CPS 1
+#endif
+constexpr int RR_MAXRING = MHS_RR_RINGCAP;
 
 template <typename T>
 struct RRP {
@@ -219,9 +225,9 @@ bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void*
     for (; G >= 1; G >>= 1) {
         const size_t slot = (size_t)(2 * RC * G + 3) * f.sx * sizeof(T);
         nring = (int)std::min<size_t>(RR_MAXRING, (limit - 128) / slot);
-        if (nring >= 3) break;
+        if (nring >= std::min(3, RR_MAXRING)) break;
     }
-    if (G < 1 || nring < 3) return false;
+    if (G < 1 || nring < std::min(3, RR_MAXRING)) return false;
     auto kern = k_resid_restrict_ring<T>;
     static PerDevice attr;
     per_device(attr, c, [&] {
@@ -239,7 +245,7 @@ bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void*
     p.ntiles = (co.sy - 1 + RC * G - 1) / (RC * G);
     const int planes = co.nz - 2;
     // z-chunks: one CTA per SM, no chunk shorter than 4 coarse planes (2 n + 3 fine planes are read for n)
-    p.nzc = std::max(1, std::min(planes / 4 > 0 ? planes / 4 : 1, c->num_sms / p.ntiles));
+    p.nzc = std::max(1, std::min(planes / 4 > 0 ? planes / 4 : 1, c->num_sms * MHS_RR_CPS / p.ntiles));
     p.down = down;
     const size_t smem = 128 + (size_t)nring * (2 * RC * G + 3) * f.sx * sizeof(T) + 16;   // (+ the element after the last row)
     launch_pdl(c, kern, dim3((unsigned)(p.ntiles * p.nzc)), dim3((unsigned)(ncx * G)), smem, p, (const T*)u, (T*)rc, done);
