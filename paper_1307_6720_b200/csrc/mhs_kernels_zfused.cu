@@ -92,6 +92,9 @@ struct ZP {
     int in_plane;       // elements of one ring slot: (WY*ZR + 2) rows x TC (also the size of an exchange plane)
     int coef_bytes;     // bytes reserved for the coefficient table (multiple of 128)
     int qb[ZQB];        // CTA b works on the items [qb[b], qb[b+1]) of the linearised (tile, plane) list (zpartition)
+    int useg, nunits;   // useg > 0: "unit" mode instead -- every tile is cut into the same useg z-segments, unit u = (segment
+                        // u / ntiles, tile u % ntiles), CTA b takes the units b, b + gridDim.x, ...: y-neighbouring tiles are walked
+                        // through the same planes at the same time (zcfg_make, "aligned segments")
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -842,11 +845,24 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     int cring = 0;                                          // coarse planes requested so far (PRO)
     const long long q0 = p.qb[blockIdx.x], q1 = p.qb[blockIdx.x + 1];
 
-    for (long long q = q0; q < q1;) {
-        const int tile = (int)(q / p.NP);
-        const int kb = 1 + (int)(q - (long long)tile * p.NP);
-        const int ke = (int)min((long long)p.NP + 1, kb + (q1 - q));   // output planes [kb, ke)
-        q += ke - kb;
+    const int ntiles_all = p.ntx * p.nty;
+    int unit = (int)blockIdx.x;
+    for (long long q = q0;;) {
+        int tile, kb, ke;                                              // output planes [kb, ke) of tile `tile`
+        if (p.useg > 0) {
+            if (unit >= p.nunits) break;
+            const int seg = unit / ntiles_all;
+            tile = unit - seg * ntiles_all;
+            kb = 1 + (int)((long long)p.NP * seg / p.useg);
+            ke = 1 + (int)((long long)p.NP * (seg + 1) / p.useg);
+            unit += (int)gridDim.x;
+        } else {
+            if (q >= q1) break;
+            tile = (int)(q / p.NP);
+            kb = 1 + (int)(q - (long long)tile * p.NP);
+            ke = (int)min((long long)p.NP + 1, kb + (q1 - q));
+            q += ke - kb;
+        }
         const int ty = tile / p.ntx, tx = tile - ty * p.ntx;
         const int ct = p.ntx == 1 ? 0 : tx * p.COUT - V;              // first column of the tile
         // Tiles along y: patch rows [jt, jt+NR) are interior rows; the wall rows j = 0 / j = sy are only ever
@@ -978,6 +994,7 @@ struct ZCfg {
     bool ok = false;
     int WX = 0, WY = 0, TC = 0, COUT = 0, ntx = 1, STEP = 0, nty = 0, ctas = 0, zcap = 0, in_plane = 0, coef_bytes = 0;
     size_t smem = 0;
+    int useg = 0, nunits = 0;      // unit mode (aligned z-segments), see ZP
     int qb[ZQB];
 };
 
@@ -1077,12 +1094,33 @@ static ZCfg zcfg_make(const mhs_ctx* c, const Level& lv, int S, bool zero, bool 
     // ranges: 147 MB read instead of 191 MB, plain pass 57.6 -> 51.1 us although every CTA runs 42 steps instead of 39 and
     // 15 SMs idle; 114 CTAs = 19 x 6: 58.4 us.  The prolongation-fused pass is bound by issue, not by DRAM, and loses
     // (78.4 -> 80.1 us): it keeps the cost-balanced ranges over all SMs.
-    if (!pro) {
-        const int ntiles = z.ntx * z.nty;
-        const int seg = ntiles > 0 ? z.ctas / ntiles : 0;
-        if (seg >= 1 && ntiles * seg * 100 >= 85 * z.ctas && (lv.nz - 2) / seg >= 16) z.ctas = ntiles * seg;
+    // More tiles than SMs (513^3: 111): the same idea in rounds -- tiles x segments units, a multiple of the CTA count, CTA b
+    // takes the units b, b + CTAs, ...; the units of one round are consecutive tiles of one z-slab (unit mode of the kernel).
+    // The segment count is the one with the least plane steps per CTA.  Measured at 513^3 (111 tiles x 4 segments = 3 rounds of
+    // 148): 478 -> 442 us per 2-sweep pass, 291.7 -> 304.6 V-cycles/s.
+    int longest = 0;
+    z.useg = 0; z.nunits = 0;
+    if (!pro && !getenv("MHS_NO_ALIGN")) {
+        const int ntiles = z.ntx * z.nty, NP = lv.nz - 2, W = 2 * S + 2;
+        long long best_cost = -1;
+        int best_seg = 0, best_ctas = 0;
+        for (int seg = 1; seg <= NP / 16; ++seg) {
+            const long long units = (long long)ntiles * seg;
+            const int rounds = (int)((units + z.ctas - 1) / z.ctas);
+            const int ctas = (int)((units + rounds - 1) / rounds);
+            if (ctas * 100 < 85 * z.ctas) continue;                     // too many idle SMs
+            if (sizeof(T) == 4 && rounds > 1) continue;                 // (fp32 passes are bound by issue: measured 1 % slower in rounds)
+            const long long cost = (long long)rounds * ((NP + seg - 1) / seg + W);
+            if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = seg; best_ctas = ctas; }
+        }
+        // against the cost-balanced ranges: NP * ntiles / CTAs planes + ~1.5 warm-ups; aligned reads pay for ~12 % more steps
+        const long long flat = ((long long)NP * ntiles + z.ctas - 1) / z.ctas + (3 * W) / 2;
+        if (best_seg > 0 && best_cost * 100 <= flat * 112) {
+            z.useg = best_seg; z.nunits = ntiles * best_seg; z.ctas = best_ctas;
+            longest = (NP + best_seg - 1) / best_seg;
+        }
     }
-    const int longest = zpartition(z.ntx * z.nty, lv.nz - 2, 2 * S + 2, z.ctas, z.qb);
+    if (!z.useg) longest = zpartition(z.ntx * z.nty, lv.nz - 2, 2 * S + 2, z.ctas, z.qb);
     z.zcap = (int)std::min<long long>(lv.nz + 1, (long long)longest + 2 * S + 3);
     z.coef_bytes = (int)(((size_t)(z.zcap + 1) * NCO * sizeof(T) + 127) / 128 * 128);
     z.in_plane = (NR + 2) * z.TC;
@@ -1128,7 +1166,11 @@ static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const voi
     p.in_plane = z.in_plane;
     p.coef_bytes = z.coef_bytes;
     p.ec = (const T*)ec; p.csp = csp;
-    for (int i = 0; i <= z.ctas; ++i) p.qb[i] = z.qb[i];
+    p.useg = z.useg; p.nunits = z.nunits;
+    if (!z.useg)
+        for (int i = 0; i <= z.ctas; ++i) p.qb[i] = z.qb[i];
+    else
+        p.qb[0] = p.qb[1] = 0;
     if (z.ntx > 1) c->prof.xtiled_zsweep += 1;
     launch_pdl(c, kern, dim3(z.ctas), dim3(WXT * ZV<T>::WY * 32), z.smem, p, (const T*)u, (const T*)rhs, (T*)out, c->partial, done);
     if (c->debug) {
