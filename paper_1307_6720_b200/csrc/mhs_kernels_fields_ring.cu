@@ -221,18 +221,24 @@ bool fr_launch(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, voi
     if (!(sx == 32 || sx == 64 || sx == 128 || sx == 256 || sx == 512 || sx == 1024) || lv.sy < 8 || lv.nz < 5) return false;
     const int G = std::max(1, 512 / sx);
     const size_t limit = 227 * 1024 - 1024;
-    // rows per strip: as many as the shared memory takes (<= 8), then the count that fills the SMs best
-    int best = 0;
+    // rows per strip (<= 8, as many as the shared memory takes) and z-chunks: the pair that keeps the SMs busiest over whole
+    // waves of CTAs (one CTA per SM: the rings take most of the shared memory), then the one with the least halo
+    int best = 0, best_nzc = 1;
     double bscore = -1.0;
     for (int R = 2; R <= 8; ++R) {
         const size_t smem = 128 + ((size_t)FR_NP * (R + 4) * sx + (size_t)FR_NB * ((R + 2) * sx + 2)) * sizeof(T);
         if (smem > limit) break;
         if ((R + G - 1) / G > FR_NRO || (R + 2 + G - 1) / G > FR_NRB) break;
         const int ns = (lv.sy - 1 + R - 1) / R;
-        const int nzc = std::max(1, std::min((lv.nz - 2) / 8 > 0 ? (lv.nz - 2) / 8 : 1, c->num_sms / ns));
-        const double fill = std::min(1.0, (double)ns * nzc / c->num_sms);
-        const double score = fill * R / (R + 4.0) + 0.2 * fill;      // occupancy first, then less halo
-        if (score > bscore) { bscore = score; best = R; }
+        const int maxc = std::max(1, (lv.nz - 2) / 16);
+        for (int nzc = 1; nzc <= maxc; ++nzc) {
+            const long long ctas = (long long)ns * nzc;
+            const long long waves = (ctas + c->num_sms - 1) / c->num_sms;
+            const double eff = (double)ctas / (double)(waves * c->num_sms);
+            const double len = (double)(lv.nz - 2) / nzc;
+            const double score = eff * (R / (R + 4.0) + 0.2) * (len / (len + 3.0));    // 3 warm-up planes per chunk
+            if (score > bscore + 1e-9) { bscore = score; best = R; best_nzc = nzc; }
+        }
     }
     if (!best) return false;
     FRP<T> q;
@@ -244,7 +250,7 @@ bool fr_launch(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, voi
     q.ft = (const T*)c->prof_tab;
     q.R = best; q.G = G;
     q.nstrips = (lv.sy - 1 + best - 1) / best;
-    q.nzc = std::max(1, std::min((lv.nz - 2) / 8 > 0 ? (lv.nz - 2) / 8 : 1, c->num_sms / q.nstrips));
+    q.nzc = best_nzc;
     const size_t smem = 128 + ((size_t)FR_NP * (best + 4) * sx + (size_t)FR_NB * ((best + 2) * sx + 2)) * sizeof(T);
     const long long N = lv.npts();
     T* Bp = (T*)B;
