@@ -195,7 +195,7 @@ bool zsweep_ok(const mhs_ctx* c, const Level& lv);
 int launch_zsweep(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, bool zero, bool norm, const int* done);
 
 // the same applied to u + P e_c (prolongation + correction folded into the pass; u is not modified).  false: not launched
-// (the level's tiles are not full rows) -- the caller prolongs separately.
+// (the level cannot run in k_zsweep) -- the caller prolongs separately.
 bool launch_zsweep_prolong(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, const Level& coarse, const void* ec,
                            const int* done);
 

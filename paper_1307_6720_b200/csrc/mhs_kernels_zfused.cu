@@ -54,9 +54,14 @@ template <typename T, int WXT> struct ZG {
     static constexpr int TC = WXT * 32 * ZV<T>::N;          // tile columns
     static constexpr int INP = (ZWY * ZR + 2) * TC;         // elements of one ring slot / exchange plane
     // prolongation-fused variant (full-row tiles only): the coarse rows under the ZWY*ZR+2 fine rows of a tile
-    static constexpr int CSX = TC / 2;                      // coarse row pitch
+    // The coarse rows come in row by row (one bulk copy each), from the 16-byte aligned coarse column at or below the one
+    // under the tile's first column (an x-tile starts one vector left of its output columns, i.e. at an odd coarse column in
+    // fp64): CPAD more elements per row than the TC/2 + 1 the tile needs at most
+    // (x-tiled variant, XT; full-row tiles -- one contiguous chunk of CROWS rows per coarse plane -- keep the plain pitch TC/2)
+    static constexpr int CPAD = 16 / (int)sizeof(T);
     static constexpr int CROWS = ZWY * ZR / 2 + 2;
-    static constexpr int CINP = CROWS * CSX + 16 / (int)sizeof(T);   // + the element after the last row (16-byte granule)
+    template <bool XT> static constexpr int csx_v = XT ? TC / 2 + CPAD : TC / 2;             // coarse row pitch in shared memory
+    template <bool XT> static constexpr int cinp_v = XT ? CROWS * (TC / 2 + CPAD) : CROWS * (TC / 2) + CPAD;   // (+ the element after the last row)
 };
 constexpr int ZQB = 200;   // capacity of the work partition table: at most ZQB-1 CTAs
 constexpr int ZNIN = 4;   // input ring depth (planes); 3 in the prolongation-fused variant (shared memory pays for the coarse ring)
@@ -309,6 +314,7 @@ struct ZCtx {
     uint32_t ce_own;              // byte offset, inside a coarse slot, of (coarse row jrow0>>1, coarse column of element 0)
     int czoff, cnext;             // ring position of coarse plane K is czoff + K; next coarse plane to request
     int jt, Jb;                   // first patch row of the tile (always odd); first coarse row held in a coarse slot
+    int cbase;                    // first coarse column held in a coarse slot
     uint32_t c0a, c1a;            // this step's two coarse planes (shared-space addresses), set by z_prolong
     // ring positions kept incrementally (a ring of 3 would otherwise cost a division per use and step):
     int rs;                       // ring slot of plane t (== (zoff + t) % NIN), rp: its mbarrier parity
@@ -351,23 +357,30 @@ __device__ __forceinline__ void z_issue(const ZP<T>& p, const T* tile_src, uint3
 // Prolongation-fused variant, warp 0: make sure every coarse plane up to the one fine plane `kfine` needs has been requested.
 // Coarse plane K (rows Jb .. Jb+CROWS-1, contiguous: full-row tiles) goes to coarse slot (czoff + K) % ZNCE; its mbarrier
 // follows the NIN barriers of the input ring.
-template <typename T, int WXT, int NIN>
+template <typename T, int WXT, int NIN, int PRO>
 __device__ __forceinline__ void c_request(const ZP<T>& p, ZCtx<T>& z, int kfine)
 {
-    constexpr int CINP = ZG<T, WXT>::CINP, CSX = ZG<T, WXT>::CSX;
+    constexpr int CINP = ZG<T, WXT>::template cinp_v<PRO == 2>, CSX = ZG<T, WXT>::template csx_v<PRO == 2>;
     if (threadIdx.x >= 32) return;      // (cnext lives in warp 0)
     const int klast = min(min(kfine, z.kend_in), p.nz - 2);
     if (klast < 1) return;
     const int kneed = (klast + 1) >> 1;
     while (z.cnext <= kneed) {
-        if (threadIdx.x == 0) {
+        {
             const int cpos = z.czoff + z.cnext;
             const int slot = cpos % ZNCE;
             uint64_t* bar = reinterpret_cast<uint64_t*>(__cvta_shared_to_generic(z.bars)) + NIN + slot;
             T* dst = reinterpret_cast<T*>(__cvta_shared_to_generic(z.ce_base)) + (size_t)slot * CINP;
-            const T* src = p.ec + p.csp * z.cnext + (long long)CSX * z.Jb;
-            mbar_expect_tx(bar, (uint32_t)(CINP * sizeof(T)));
-            bulk_g2s(dst, src, (uint32_t)(CINP * sizeof(T)), bar);
+            const T* src = p.ec + p.csp * z.cnext + (long long)(p.sx >> 1) * z.Jb + (PRO == 2 ? z.cbase : 0);
+            const int lane = (int)threadIdx.x;
+            if (PRO == 2) {      // x-tiles: the coarse rows under the tile are not contiguous -- one copy per row
+                if (lane == 0) mbar_expect_tx(bar, (uint32_t)(CINP * sizeof(T)));
+                __syncwarp();
+                if (lane < ZG<T, WXT>::CROWS) bulk_g2s(dst + lane * CSX, src + (long long)lane * (p.sx >> 1), (uint32_t)(CSX * sizeof(T)), bar);
+            } else if (lane == 0) {
+                mbar_expect_tx(bar, (uint32_t)(CINP * sizeof(T)));
+                bulk_g2s(dst, src, (uint32_t)(CINP * sizeof(T)), bar);
+            }
         }
         ++z.cnext;
     }
@@ -395,7 +408,7 @@ __device__ __forceinline__ void zc_load(ZCoef<float>& k, uint32_t a, bool, bool)
 }
 
 // End of a plane step: the ring slot of plane t-1 and the exchange plane of t-2 have been read by everybody.
-template <typename T, int WXT, bool ZERO, bool PRO>
+template <typename T, int WXT, bool ZERO, int PRO>
 __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, bool may_issue)
 {
     constexpr int NIN = PRO ? 3 : ZNIN;
@@ -405,7 +418,7 @@ __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* t
         if (k <= z.kend_in) {
             // (zoff + k) % NIN is the slot of plane t-1
             if (threadIdx.x < 32) z_issue<T, WXT, NIN>(p, tile_src, z.bars, IN, z.rs == 0 ? NIN - 1 : z.rs - 1, k);
-            if (PRO) c_request<T, WXT, NIN>(p, z, k + 1);   // (one plane ahead: the coarse plane is there when its fine plane lands)
+            if (PRO) c_request<T, WXT, NIN, PRO>(p, z, k + 1);   // (one plane ahead: the coarse plane is there when its fine plane lands)
         }
     }
     ++z.t;
@@ -423,13 +436,13 @@ __device__ __forceinline__ void z_advance(const ZP<T>& p, ZCtx<T>& z, const T* t
 // columns only (walls and the planes k = 0, nz-1 carry no correction).  Coarse operands come from the coarse ring.
 //   u(i,j,k) += 1/8 * sum over the 2x2x2 coarse nodes ((i,i+1)>>1, (j,j+1)>>1, (k,k+1)>>1)
 // ------------------------------------------------------------------------------------------------
-template <typename T, int WXT, int JP>
+template <typename T, int WXT, int JP, int PRO>
 __device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, uint32_t c0a, uint32_t c1a)
 {
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N, VC = V / 2;
     constexpr uint32_t ES = sizeof(T);
-    constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES, crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
+    constexpr uint32_t rowb = (uint32_t)ZG<T, WXT>::TC * ES, crowb = (uint32_t)ZG<T, WXT>::template csx_v<PRO == 2> * ES;
     constexpr int NJ = (JP + ZR) / 2 + 1;          // coarse rows under the ZR patch rows
     T cz[NJ][VC + 1];                              // the two coarse planes summed
 #pragma unroll
@@ -453,15 +466,15 @@ __device__ __forceinline__ void z_prolong_rows(const ZCtx<T>& z, uint32_t a_pl, 
     }
 }
 
-template <typename T, int WXT, int NIN, bool ROWS = true>
+template <typename T, int WXT, int NIN, bool ROWS, int PRO>
 __device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int slot)
 {
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int V = ZV<T>::N, VC = V / 2;
     constexpr uint32_t ES = sizeof(T);
     constexpr int TC = ZG<T, WXT>::TC, NR = ZWY * ZR;
-    constexpr uint32_t planeb = (uint32_t)ZG<T, WXT>::INP * ES, cplaneb = (uint32_t)ZG<T, WXT>::CINP * ES;
-    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * ES;
+    constexpr uint32_t planeb = (uint32_t)ZG<T, WXT>::INP * ES, cplaneb = (uint32_t)ZG<T, WXT>::template cinp_v<PRO == 2> * ES;
+    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::template csx_v<PRO == 2> * ES;
     z.corr = false;
     if (t < 1 || t > p.nz - 2) return;
     z.corr = true;
@@ -477,7 +490,7 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int
     const uint32_t c0a = z.ce_base + (uint32_t)s0 * cplaneb, c1a = z.ce_base + (uint32_t)s1 * cplaneb;
     const uint32_t a_pl = z.in_own + (uint32_t)slot * planeb;
     z.c0a = c0a; z.c1a = c1a;
-    if (ROWS) z_prolong_rows<T, WXT, 1>(z, a_pl, c0a, c1a);     // (jt is odd and patch rows start ZR-aligned from it)
+    if (ROWS) z_prolong_rows<T, WXT, 1, PRO>(z, a_pl, c0a, c1a);     // (jt is odd and patch rows start ZR-aligned from it)
     // the halo rows of the tile (fine rows jt-1 and jt+NR): one vector per thread (which one: fixed per segment, z.h_*)
     if (z.h_ok) {
         const uint32_t a = z.in_base + (uint32_t)slot * planeb + z.h_a;
@@ -500,14 +513,14 @@ __device__ __forceinline__ void z_prolong(const ZP<T>& p, ZCtx<T>& z, int t, int
 }
 
 // First step of a segment (t = kstart): nothing to compute yet, plane kstart becomes the centre plane.
-template <typename T, int WXT, bool ZERO, bool PRO>
+template <typename T, int WXT, bool ZERO, int PRO>
 __device__ __forceinline__ void z_first(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0)
 {
     constexpr int ZR = ZV<T>::R, ZWY = ZV<T>::WY; (void)ZR; (void)ZWY;
     constexpr int NIN = PRO ? 3 : ZNIN;
     if (!ZERO) {
         mbar_wait32(z.bars + 8 * z.rs, z.rp);
-        if (PRO) z_prolong<T, WXT, NIN>(p, z, z.t, z.rs);
+        if (PRO) z_prolong<T, WXT, NIN, true, PRO>(p, z, z.t, z.rs);
         const uint32_t a = z.in_own + (uint32_t)z.rs * (uint32_t)(ZG<T, WXT>::INP * sizeof(T));
 #pragma unroll
         for (int r = 0; r < ZR; ++r) dn0.r[r] = lds_vec<T>(a + r * (uint32_t)(ZG<T, WXT>::TC * sizeof(T)));
@@ -533,7 +546,7 @@ __device__ __forceinline__ void norm_acc(double& pa, double& pb, double d0, doub
 // the 64 register moves per step that `dn0 = up; dn1 = o1` used to cost are gone.
 // A wall column (element 0 of the first vector of a row) stays exactly zero through its coefficients: its own value and its
 // z- and y-neighbours are walls (zero), so with By = wz = 0 for that element the update returns 0 -- no select per row.
-template <int WXT, int S, bool HAS_RHS, bool NORM, bool PRO, bool ISO>
+template <int WXT, int S, bool HAS_RHS, bool NORM, int PRO, bool ISO>
 __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, const ZCoef<double>& k1, const ZCoef<double>& k2, Patch<double>& dn0,
                                          const Patch<double>& c0, Patch<double>& dn1, const Patch<double>& c1, uint32_t a_new, uint32_t a_cen,
                                          uint32_t a_exw, uint32_t a_exr, int m1, int m2, double& pa)
@@ -583,7 +596,7 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
     // prolongation-fused variant: the two coarse planes of this step summed, per coarse row under the patch (loaded as needed);
     // planes without a correction (k = 0, nz-1, the idle step) run the same code with the weights 0 on whatever finite
     // numbers the coarse ring holds (it is zero-filled at the start of the kernel)
-    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * 8u;
+    constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::template csx_v<PRO == 2> * 8u;
     T cz[ZR / 2 + 1][2], czr[ZR / 2 + 1][4];
     ZVec<T> upb[2];           // plane t of the rows r, r+1 as loaded (uncorrected), two rows ahead of their correction
     const T cs1 = (PRO && z.corr) ? 0.125 : 0.0, cs2 = (PRO && z.corr) ? 0.25 : 0.0;
@@ -659,7 +672,7 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
 // One plane step, t > kstart.  Input planes of the patch: dn0 = t-2, c0 = t-1 (plane t is read from its ring
 // slot); sweep-1 planes: dn1 = t-3, c1 = t-2.  On return dn0 holds plane t and dn1 holds sweep-1 plane t-1: the
 // caller swaps the names (steps come in pairs).
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO, bool ISO>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, int PRO, bool ISO>
 __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile_src, T* IN, Patch<T>& dn0, const Patch<T>& c0, Patch<T>& dn1,
                                        const Patch<T>& c1)
 {
@@ -680,7 +693,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     const uint32_t a_exr = z.ex_own + (uint32_t)((t & 1) ^ 1) * planeb;                // sweep-1 plane t-2 (written a step ago)
     if (fresh) mbar_wait32(z.bars + 8 * z.rs, z.rp);
     if (PRO) z.corr = false;
-    if (PRO && fresh) z_prolong<T, WXT, NIN, sizeof(T) == 4>(p, z, t, z.rs);   // fp64: own rows inside the row loop
+    if (PRO && fresh) z_prolong<T, WXT, NIN, sizeof(T) == 4, PRO>(p, z, t, z.rs);   // fp64: own rows inside the row loop
     ZCoef<T> k1, k2;
     zc_load(k1, z.coef, HAS_RHS, NORM);
     if (S == 2) zc_load(k2, z.coef - ZV<T>::NCO * ES, HAS_RHS, false);
@@ -786,7 +799,7 @@ __device__ __forceinline__ void z_step(const ZP<T>& p, ZCtx<T>& z, const T* tile
     z_advance<T, WXT, ZERO, PRO>(p, z, tile_src, IN, true);
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO, bool ISO>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, int PRO, bool ISO>
 __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid_constant__ ZP<T> p, const T* __restrict__ u, const T* __restrict__ rhs,
                                                     T* __restrict__ out, double* __restrict__ partial, const int* __restrict__ done)
 {
@@ -822,7 +835,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     }
     if (threadIdx.x < NCO) coef[-NCO + (int)threadIdx.x] = T(0);
     if (PRO) {   // (planes without a correction read the coarse ring with zero weights: finite numbers, please)
-        for (int q = threadIdx.x; q < ZNCE * ZG<T, WXT>::CINP; q += blockDim.x) CE[q] = T(0);
+        for (int q = threadIdx.x; q < ZNCE * ZG<T, WXT>::template cinp_v<PRO == 2>; q += blockDim.x) CE[q] = T(0);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes before the bulk copies into the same memory
     }
     __syncthreads();
@@ -838,7 +851,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
     z.eo2 = z.swp ? (uint32_t)(0u - (uint32_t)sizeof(T)) : (uint32_t)(V * sizeof(T));
     z.in_base = smem_u32(IN);
     z.ce_base = PRO ? smem_u32(CE) : 0u;
-    z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0;
+    z.ce_own = 0; z.czoff = 0; z.cnext = 0; z.jt = 0; z.Jb = 0; z.cbase = 0;
     z.c0a = z.c1a = z.ce_base; z.corr = false; z.wrow = false;
     z.rs = 0; z.rp = 0; z.cs0 = 0; z.cp0 = 0; z.h_ok = false; z.h_a = z.h_co = z.h_dj = 0; z.h_c0 = false;
     int ring = 0;                                           // planes requested so far by this CTA (ring position)
@@ -909,6 +922,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
                 z.kend_in = kend_in;
                 z.jt = jt;
                 z.Jb = (jt - 1) >> 1;
+                z.cbase = PRO == 2 ? (ct >> 1) & ~(ZG<T, WXT>::CPAD - 1) : 0;
                 const int kfirst = max(kstart, 1), klast = min(kend_in, p.nz - 2);
                 z.cnext = kfirst >> 1;
                 z.czoff = cring - z.cnext;
@@ -918,17 +932,18 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
                     z.cp0 = (uint32_t)((p0 / ZNCE) & 1);
                 }
                 if (klast >= kfirst) cring += ((klast + 1) >> 1) - z.cnext + 1;
-                c_request<T, WXT, NIN>(p, z, kstart + n);
+                c_request<T, WXT, NIN, PRO>(p, z, kstart + n);
                 // the halo vector this thread corrects: row jt-1 (threads 0 .. TC/V-1) or row jt+NR (the next TC/V threads)
                 constexpr int nvr = TC / V;
-                constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::CSX * sizeof(T);
+                constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::template csx_v<PRO == 2> * sizeof(T);
                 const int which = (int)threadIdx.x / nvr, hv = (int)threadIdx.x - which * nvr;
                 const int jh = which ? jt + NR : jt - 1;
                 z.h_ok = which < 2 && jh >= 1 && jh < p.sy;
                 z.h_a = (uint32_t)(((which ? NR + 1 : 0) * TC + hv * V) * (int)sizeof(T));
-                z.h_co = (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)sizeof(T));
+                z.h_co = PRO == 2 ? (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + (((ct + hv * V) >> 1) - z.cbase) * (int)sizeof(T))
+                                  : (uint32_t)(((jh >> 1) - z.Jb) * (int)crowb + ((hv * V) >> 1) * (int)sizeof(T));
                 z.h_dj = (jh & 1) ? crowb : 0u;
-                z.h_c0 = hv == 0;
+                z.h_c0 = PRO == 2 ? (ct + hv * V == 0 || ct + hv * V == p.sx) : hv == 0;
             }
         }
         __syncthreads();   // coefficient table visible
@@ -951,7 +966,7 @@ __global__ void __launch_bounds__(WXT * ZV<T>::WY * 32, 1) k_zsweep(const __grid
         z.kb = kb;
         z.nout = ke - kb;
         z.kend_in = kend_in;
-        if (PRO) z.ce_own = (uint32_t)((((jrow0 >> 1) - z.Jb) * ZG<T, WXT>::CSX + (icol0 >> 1)) * (int)sizeof(T));
+        if (PRO) z.ce_own = (uint32_t)((((jrow0 >> 1) - z.Jb) * ZG<T, WXT>::template csx_v<PRO == 2> + ((icol0 >> 1) - (PRO == 2 ? z.cbase : 0))) * (int)sizeof(T));
         z.coef = smem_u32(coef);
         // the first z_step runs at t = kstart+1: sweep 1 makes plane kstart, sweep 2 plane kstart-1
         z.f1 = rhs + own + p.sp * kstart;
@@ -1127,16 +1142,17 @@ static ZCfg zcfg_make(const mhs_ctx* c, const Level& lv, int S, bool zero, bool 
     const size_t plane = (size_t)z.in_plane * sizeof(T);
     const size_t limit = 227 * 1024 - 256;   // the kernel also has a little static shared memory
     z.smem = 128 + z.coef_bytes + (zero ? 0 : (pro ? 3 : ZNIN) * plane) + 2 * plane;
-    if (pro) {   // full-row tiles only: the coarse rows under a tile are then one contiguous chunk per plane
-        if (z.ntx != 1 || zero) return z;
-        z.smem += (size_t)ZNCE * (((NR / 2 + 2) * (z.TC / 2) + 16 / sizeof(T)) * sizeof(T));
+    if (pro) {   // the coarse rows under a tile: a ring of ZNCE coarse planes of NR/2 + 2 rows
+        if (zero) return z;
+        const size_t cpad = 16 / sizeof(T);
+        z.smem += (size_t)ZNCE * (z.ntx == 1 ? (NR / 2 + 2) * (z.TC / 2) + cpad : (NR / 2 + 2) * (z.TC / 2 + cpad)) * sizeof(T);
     }
     if (z.smem > limit) return z;
     z.ok = true;
     return z;
 }
 
-template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, bool PRO = false, bool ISO = false>
+template <typename T, int WXT, int S, bool HAS_RHS, bool ZERO, bool NORM, int PRO = 0, bool ISO = false>
 static int zsweep_launch_w(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done,
                            const void* ec = nullptr, long long csp = 0)
 {
@@ -1197,16 +1213,21 @@ template <typename T, int S, bool HAS_RHS>
 static void zsweep_launch_pro(mhs_ctx* c, const Level& lv, const ZCfg& z, const void* u, const void* rhs, void* out, const int* done,
                               const void* ec, long long csp)
 {
+    if (z.ntx > 1) {     // x-tiles (3 or 4 warps wide): the variant whose coarse rows come in row by row (PRO = 2)
+        if (z.WX == 3) zsweep_launch_w<T, 3, S, HAS_RHS, false, false, 2>(c, lv, z, u, rhs, out, done, ec, csp);
+        else zsweep_launch_w<T, 4, S, HAS_RHS, false, false, 2>(c, lv, z, u, rhs, out, done, ec, csp);
+        return;
+    }
     switch (z.WX) {
-        case 1: zsweep_launch_w<T, 1, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
-        case 2: zsweep_launch_w<T, 2, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
-        case 3: zsweep_launch_w<T, 3, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
-        default: zsweep_launch_w<T, 4, S, HAS_RHS, false, false, true>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        case 1: zsweep_launch_w<T, 1, S, HAS_RHS, false, false, 1>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        case 2: zsweep_launch_w<T, 2, S, HAS_RHS, false, false, 1>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        case 3: zsweep_launch_w<T, 3, S, HAS_RHS, false, false, 1>(c, lv, z, u, rhs, out, done, ec, csp); break;
+        default: zsweep_launch_w<T, 4, S, HAS_RHS, false, false, 1>(c, lv, z, u, rhs, out, done, ec, csp); break;
     }
 }
 
 // S (1 or 2) sweeps of level lv applied to u + P e_c (e_c = co's iterate `ec`): the trilinear correction is folded into the
-// pass, u itself is not modified.  Returns false (nothing launched) when the level's tiles are not full rows.
+// pass, u itself is not modified.  Returns false (nothing launched) when the level cannot run in k_zsweep at all.
 bool launch_zsweep_prolong(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int S, const Level& co, const void* ec,
                            const int* done)
 {
