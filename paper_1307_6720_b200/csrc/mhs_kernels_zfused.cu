@@ -598,7 +598,6 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
     // numbers the coarse ring holds (it is zero-filled at the start of the kernel)
     constexpr uint32_t crowb = (uint32_t)ZG<T, WXT>::template csx_v<PRO == 2> * 8u;
     T cz[ZR / 2 + 1][2], czr[ZR / 2 + 1][4];
-    ZVec<T> upb[2];           // plane t of the rows r, r+1 as loaded (uncorrected), two rows ahead of their correction
     const T cs1 = (PRO && z.corr) ? 0.125 : 0.0, cs2 = (PRO && z.corr) ? 0.25 : 0.0;
     const uint32_t cb0 = z.c0a + z.ce_own, cb1 = z.c1a + z.ce_own;
     auto czload = [&](int q) {    // (issued well ahead of czsum: a store to shared memory sits between every two rows, and no
@@ -622,10 +621,12 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
             if (r == 0) { czsum(0); czsum(1); }
             else if (q1 != q0) czsum(q1);
             const T e0 = cz[q0][0] + cz[q1][0], e1 = cz[q0][1] + cz[q1][1];
-            dn0.r[r].v[0] = fma(cs2, e0, upb[r & 1].v[0]);
-            dn0.r[r].v[1] = fma(cs1, e0 + e1, upb[r & 1].v[1]);
+            // (the plane's row loaded two rows ahead of this point into a buffer of its own bought nothing -- 82.8 -> 82.4 us --
+            //  and cost eight registers: 64 bytes of spills in the x-tiled variant)
+            const ZVec<T> raw = lds_vec<T>(a_new + r * rowb);
+            dn0.r[r].v[0] = fma(cs2, e0, raw.v[0]);
+            dn0.r[r].v[1] = fma(cs1, e0 + e1, raw.v[1]);
             sts_vec(a_new + r * rowb, dn0.r[r]);
-            if (r + 2 < ZR) upb[r & 1] = lds_vec<T>(a_new + (r + 2) * rowb);
             if (r + 2 < ZR && ((4 + r) >> 1) != ((3 + r) >> 1)) czload((4 + r) >> 1);      // the coarse row that row r+2 adds
         }
         if (S == 2) {
@@ -636,8 +637,6 @@ __device__ __forceinline__ void z_rows64(const ZP<double>& p, ZCtx<double>& z, c
     };
     double pn[4] = {0.0, 0.0, 0.0, 0.0};     // four partial sums of the norm: dependency chains of 4 FMAs instead of 16
     if (PRO) {
-        upb[0] = lds_vec<T>(a_new);
-        upb[1] = lds_vec<T>(a_new + rowb);
         czload(0); czload(1);                  // (row r+2's new coarse row is requested while row r is corrected)
     }
     load_nb(0, nb[0]);
