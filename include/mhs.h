@@ -271,6 +271,24 @@ mhs_status mhs_op_vcycle(mhs_ctx *ctx, int dim, int level);               /* one
                                                                              from u = 0 as inside a cycle      */
 mhs_status mhs_op_resnorm(mhs_ctx *ctx, int dim, int level, double *out_host); /* ||rhs - L u||_2     */
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the residual norm of eq 8 (the quantity of the stop rule, C10),
+ *     *out_device = || [c_k (D_xx + D_yy) + D_zz + alpha^2] P ||_2   over the interior nodes,  c_k = 1 + f(z_k) = 1 - xi(z_k),
+ * of a DENSE potential P (nx*ny*nz elements of `dtype`, device; boundary nodes included and read as they are).  It
+ * needs no mhs_ctx and calls no cudaMalloc / cudaFree or allocating library routine: its partial sums live in a
+ * file-scope device array of MHS_STATIC_SCRATCH_DOUBLES doubles (512 KB, held by every GPU that loads the library
+ * until the process exits).  One partial sum per 8 rows of a plane: grids with ceil((ny-2)/8) * (nz-2) >
+ * MHS_STATIC_SCRATCH_DOUBLES (or nz - 2 > 65535) are rejected with MHS_ERR_INVALID_ARG (513^3 needs 32704, 1025 x 1025 x 257
+ * 32640).  c_device: nz doubles on the device.  hx, hy, hz: mesh widths.  stream: a cudaStream_t (NULL = default
+ * stream); the call is asynchronous, the result is ordered on `stream`.  Every call shares the one scratch array:
+ * calls that overlap on the GPU race.  The array keeps the last call's contents; no call depends on them.
+ * mhs_static_last_error(): message of the calling thread's last failed mhs_resnorm_static.                          */
+#define MHS_STATIC_SCRATCH_DOUBLES 65536
+mhs_status mhs_resnorm_static(const void *P_device, int dtype, int nx, int ny, int nz, double hx, double hy, double hz,
+                              double alpha, const double *c_device, double *out_device, void *stream);
+const char *mhs_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -38,7 +38,9 @@ EXPORTS = [
     "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
     "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
+    "mhs_resnorm_static", "mhs_static_last_error",
 ]
+MHS_STATIC_SCRATCH_DOUBLES = 65536
 
 
 class mhs_grid(C.Structure):
@@ -124,6 +126,9 @@ def lib():
         for n in ("mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle"):
             getattr(L, n).argtypes = [vp, ip, ip]
         L.mhs_op_resnorm.argtypes = [vp, ip, ip, C.POINTER(C.c_double)]
+        L.mhs_resnorm_static.argtypes = [vp, ip, ip, ip, ip, dp, dp, dp, dp, vp, vp, vp]
+        L.mhs_static_last_error.argtypes = []
+        L.mhs_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -243,6 +248,18 @@ def mhs_get_potential(h, P, dtype, N):
 
 def mhs_set_potential(h, P, dtype, N):
     _check(h, lib().mhs_set_potential(h, _dptr(P, dtype, N)))
+
+
+def mhs_resnorm_static(P, c, out, nx, ny, nz, hx, hy, hz, alpha, stream=None):
+    """mhs_resnorm_static (include/mhs.h): ||L P||_2 of the dense device tensor P into the 1-element fp64 device tensor
+    `out`; c: nz fp64 device values 1 + f(z_k).  Allocates nothing; asynchronous on `stream` (default: torch's current)."""
+    if P.dtype not in (torch.float32, torch.float64):
+        raise TypeError("P must be float32 or float64")
+    s = torch.cuda.current_stream().cuda_stream if stream is None else stream
+    st = lib().mhs_resnorm_static(_dptr(P, P.dtype, nx * ny * nz), MHS_F64 if P.dtype == torch.float64 else MHS_F32, nx, ny, nz,
+                                  hx, hy, hz, alpha, _dptr(c, torch.float64, nz), _dptr(out, torch.float64, 1), C.c_void_p(s))
+    if st != MHS_OK:
+        raise MHSError(st, lib().mhs_static_last_error().decode())
 
 
 def mhs_get_profile(h):
