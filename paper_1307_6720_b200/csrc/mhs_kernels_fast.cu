@@ -349,7 +349,7 @@ static int pick_chunks(long long xy_blocks, int planes, int slots, int min_chunk
 
 // Levels that fit in the L2 several times over (<= ~5 M nodes: 129^3 and below) are not bandwidth problems but
 // parallelism problems: they get one row per thread and short z-chunks, so that even 65^3 fills the 148 SMs.
-bool mid_level(const mhs_ctx* c, const Level& lv) { return !(c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS) && lv.npts() <= 5000000LL; }
+bool mid_level(const mhs_ctx* c, const Level& lv) { return !(c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS) && lv.npts() <= c->mid_pts; }
 
 template <typename T, int R, bool HAS_RHS, bool STORE, bool NORM, bool ZERO2>
 static long long smooth_z_t(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int reverse, const int* done)

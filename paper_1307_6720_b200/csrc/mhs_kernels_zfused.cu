@@ -1114,7 +1114,7 @@ static ZCfg zcfg_make(const mhs_ctx* c, const Level& lv, int S, bool zero, bool 
     // 148): 478 -> 442 us per 2-sweep pass, 291.7 -> 304.6 V-cycles/s.
     int longest = 0;
     z.useg = 0; z.nunits = 0;
-    if (!pro && !getenv("MHS_NO_ALIGN")) {
+    if (!pro && !c->no_align) {
         const int ntiles = z.ntx * z.nty, NP = lv.nz - 2, W = 2 * S + 2;
         long long best_cost = -1;
         int best_seg = 0, best_ctas = 0;
