@@ -13,7 +13,7 @@ import sys
 
 from . import build as _build
 
-DEFAULT = r"k_zsweep<double, 4, 2, 0, 0, (1, 0|0, 1), 1>|k_resid_restrict_ring<double>|k_fields_ring<double, 256|k_resid_restrict_sep<double, 4, 0>|k_fields_z<double|k_zline<double, 0>|k_fieldlines<double>|k_cluster<double, 1>"
+DEFAULT = r"k_zsweep<double, 4, 2, 0, 0, (1, 0|0, 1), 1>|k_resid_restrict_ring<double>|k_fields_ring<double, 256|k_resid_restrict_sep<double, 4, 0>|k_fields_z<double|k_zline<double, 0>|k_fieldlines<double>|k_cluster<double, [01]>|k_resnorm_static_partial<double>"
 
 
 def demangle(names):
