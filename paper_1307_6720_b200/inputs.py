@@ -200,6 +200,18 @@ def random_field(shape, seed: int, zero_boundary: bool = True) -> np.ndarray:
     return a
 
 
+def wall_data(w: "Workload", amp: float = 0.3, seed: int = 0) -> np.ndarray:
+    """Dirichlet data for P on the side and top faces ("other elliptic equations can be defined on the other
+    boundaries" -- their solutions would be such data): a smooth seeded function sampled on the whole (nz, ny, nx) grid; only its
+    values on the side and top boundary nodes are used by the solver.  No method arithmetic here: just the samples."""
+    rng = SplitMix64(SEED_BASE + 5000 + seed)
+    k1, k2, k3, ph1, ph2 = (float(v) for v in rng.uniform(0.5, 2.5, 5))
+    z = np.linspace(0.0, w.Lz, w.nz)[:, None, None]
+    y = np.linspace(0.0, w.Ly, w.ny)[None, :, None]
+    x = np.linspace(0.0, w.Lx, w.nx)[None, None, :]
+    return amp * (np.sin(k1 * x / w.Lx * np.pi + ph1) * np.cos(k2 * y / w.Ly * np.pi + ph2) * np.exp(-k3 * z / w.Lz) + 0.25)
+
+
 # ------------------------------------------------------------------------------------------------
 # The paper's own examples (PAPER.md:119-156, section 3): a second, fully analytic test-bed (SURVEY 8(f) NEXT-1).
 # ------------------------------------------------------------------------------------------------
