@@ -64,8 +64,10 @@ typedef enum {
 
 typedef struct { int nx, ny, nz; double Lx, Ly, Lz; } mhs_grid;
 
-#define MHS_BC_DIRICHLET_ZERO 0
-typedef struct { int sides, top; } mhs_bc; /* only MHS_BC_DIRICHLET_ZERO: P = 0 */
+#define MHS_BC_DIRICHLET_ZERO 0 /* P = 0 on the face: the paper's choice                                     */
+#define MHS_BC_DIRICHLET_DATA 1 /* P given on the face by mhs_set_wall_data ("In principle other elliptic
+                                   equations can be defined on the other boundaries")                  */
+typedef struct { int sides, top; } mhs_bc; /* the four side faces / the top face; NULL = both MHS_BC_DIRICHLET_ZERO */
 
 #define MHS_F32 0
 #define MHS_F64 1
@@ -270,6 +272,20 @@ mhs_status mhs_op_vcycle(mhs_ctx *ctx, int dim, int level);               /* one
                                                                              continues from u, levels >= 1 start
                                                                              from u = 0 as inside a cycle      */
 mhs_status mhs_op_resnorm(mhs_ctx *ctx, int dim, int level, double *out_host); /* ||rhs - L u||_2     */
+
+/* Dirichlet data for P on the side and top faces (contexts created with MHS_BC_DIRICHLET_DATA in mhs_bc.sides and / or
+ * .top; MHS_ERR_STATE otherwise).  G_device: a DENSE nx*ny*nz array of the context's dtype (device) of which only the nodes on
+ * faces declared MHS_BC_DIRICHLET_DATA are read -- side nodes i = 0, nx-1 or j = 0, ny-1 on every plane k (the rim of the
+ * bottom plane included), top nodes k = nz-1 away from the rim; faces declared MHS_BC_DIRICHLET_ZERO keep P = 0.  The values
+ * would come from whatever problems are posed on those faces (a boundary-only context, nz = 1, solves eq 11 on a face).
+ * The data is copied; it stays in force until the next call (mhs_solve_boundary resets the interior, not the walls).  Until
+ * the first call the walls are zero.  Such a context solves  eq 8  with P = G on those faces: internally P = P_h + W, W = the
+ * wall values, P_h with zero walls and the right-hand side -L W on the finest level (it allocates that array, W and one dense
+ * scratch array in mhs_create: 3N elements more); mhs_get_potential and mhs_fields return the full P and its fields
+ * (B = 0 on side and top nodes as before, C13; the nodes next to them take the wall values through the central differences),
+ * the latter by the general one-thread-per-node kernel.  mhs_set_potential sets P_h: the wall nodes of its argument are
+ * ignored.  Needs the point-Jacobi smoother and fmg_cycles = 0 (mhs_create: MHS_ERR_INVALID_ARG otherwise).               */
+mhs_status mhs_set_wall_data(mhs_ctx *ctx, const void *G_device);
 
 /* ---- an entry point that allocates nothing ---------------------------------------------------------------------
  * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid

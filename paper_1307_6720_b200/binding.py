@@ -38,8 +38,9 @@ EXPORTS = [
     "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host", "mhs_last_error", "mhs_status_string", "mhs_get_profile", "mhs_reset_profile",
     "mhs_kernel_class_name", "mhs_set_profiling", "mhs_num_levels", "mhs_level_dims", "mhs_level_set", "mhs_level_get",
     "mhs_op_smooth", "mhs_op_residual", "mhs_op_restrict", "mhs_op_prolong", "mhs_op_vcycle", "mhs_op_resnorm",
-    "mhs_resnorm_static", "mhs_static_last_error",
+    "mhs_resnorm_static", "mhs_static_last_error", "mhs_set_wall_data",
 ]
+MHS_BC_DIRICHLET_ZERO, MHS_BC_DIRICHLET_DATA = 0, 1
 MHS_STATIC_SCRATCH_DOUBLES = 65536
 
 
@@ -107,7 +108,7 @@ def lib():
         L.mhs_host_sync.argtypes = [vp]
         L.mhs_diagnostics.argtypes = [vp, vp, vp, vp, vp]
         L.mhs_fieldlines.argtypes = [vp, vp, ip, vp, dp, ip, ip, dp, vp, vp]
-        for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host"):
+        for n in ("mhs_get_potential", "mhs_get_potential_host", "mhs_set_potential", "mhs_get_boundary", "mhs_get_boundary_host", "mhs_set_wall_data"):
             getattr(L, n).argtypes = [vp, vp]
         L.mhs_last_error.argtypes = [vp]
         L.mhs_last_error.restype = C.c_char_p
@@ -171,8 +172,8 @@ def _info(i: mhs_solve_info, status):
 # ------------------------------------------------------------------ C-named functions ---------
 def mhs_create(nx, ny, nz, Lx, Ly, Lz, alpha, f_profile=None, *, dtype=torch.float64, omega=2.0 / 3.0,
                n_pre=2, n_post=2, max_levels=0, boundary_tol=1e-10, boundary_max_cycles=100, mu0=0.5, g=1.0,
-               p_b=None, rho_b=None, dfdz=None, stream=None, profile=0, flags=0, smoother=0, fmg_cycles=0):
-    """-> opaque context handle (int).  See include/mhs.h: mhs_create."""
+               p_b=None, rho_b=None, dfdz=None, stream=None, profile=0, flags=0, smoother=0, fmg_cycles=0, bc=None):
+    """-> opaque context handle (int).  See include/mhs.h: mhs_create.  bc: None or (sides, top) of MHS_BC_*."""
     L = lib()
     if not torch.cuda.is_available():
         raise RuntimeError("no CUDA device: paper_1307_6720_b200 has no CPU fallback")
@@ -197,8 +198,9 @@ def mhs_create(nx, ny, nz, Lx, Ly, Lz, alpha, f_profile=None, *, dtype=torch.flo
     o.smoother, o.fmg_cycles = smoother, fmg_cycles
     grid = mhs_grid(nx, ny, nz, Lx, Ly, Lz)
     h = C.c_void_p()
+    bcs = mhs_bc(int(bc[0]), int(bc[1])) if bc is not None else None
     st = L.mhs_create(C.byref(grid), alpha, keep[3].ctypes.data_as(pd) if keep[3] is not None else None,
-                      None, C.byref(o), C.byref(h))
+                      C.byref(bcs) if bcs is not None else None, C.byref(o), C.byref(h))
     if st != MHS_OK:
         msg = L.mhs_last_error(h).decode() if h else ""
         if h:
@@ -260,6 +262,10 @@ def mhs_resnorm_static(P, c, out, nx, ny, nz, hx, hy, hz, alpha, stream=None):
                                   hx, hy, hz, alpha, _dptr(c, torch.float64, nz), _dptr(out, torch.float64, 1), C.c_void_p(s))
     if st != MHS_OK:
         raise MHSError(st, lib().mhs_static_last_error().decode())
+
+
+def mhs_set_wall_data(h, G, dtype, N):
+    _check(h, lib().mhs_set_wall_data(h, _dptr(G, dtype, N)))
 
 
 def mhs_get_profile(h):
@@ -395,6 +401,10 @@ class Solver:
 
     def set_potential(self, P):
         mhs_set_potential(self.h, P, self.dtype, self.N)
+
+    def set_wall_data(self, G):
+        """Dirichlet data on the faces declared MHS_BC_DIRICHLET_DATA (Solver(..., bc=(sides, top))): G dense (nz, ny, nx) device tensor."""
+        mhs_set_wall_data(self.h, G.reshape(-1), self.dtype, self.N)
 
     def profile(self):
         return mhs_get_profile(self.h)

@@ -233,7 +233,7 @@ mhs_status build_hierarchy(mhs_ctx* ctx, int dim, std::vector<Level>& Ls)
             if ((st = upload(ctx, &lv.zl, zl))) return st;
         }
         if ((st = alloc_field(ctx, lv, 0, &lv.u))) return st;
-        if (!(dim == 3 && l == 0))
+        if (!(dim == 3 && l == 0) || ctx->wall_ctx)   // (eq 8 is homogeneous: no right-hand side on the finest 3D level -- unless wall data is lifted into one)
             if ((st = alloc_field(ctx, lv, 2, &lv.rhs))) return st;
         if (!lv.coarsest) {
             if ((st = alloc_field(ctx, lv, 1, &lv.tmp))) return st;
@@ -324,7 +324,7 @@ int clus_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim
 long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const int* done, bool want_norm = false)
 {
     Level& lv = Ls[l];
-    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    const void* rhs = lv.rhs /* (finest 3D level: NULL unless wall data is lifted into it) */;
     const bool fast = use_fast(ctx, lv);
     long long npart = 0;
     if (use_zline(ctx, lv)) {    // z-line Jacobi: one tridiagonal solve per (i,j) line and sweep (no norm by-product)
@@ -367,7 +367,7 @@ long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const 
 long long resnorm_partials(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done)
 {
     Level& lv = Ls[l];
-    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    const void* rhs = lv.rhs /* (finest 3D level: NULL unless wall data is lifted into it) */;
     Scope sc(ctx, kc_for(lv, l, 3));
     if (use_fast(ctx, lv)) return launch_smooth_z(ctx, lv, lv.u, rhs, nullptr, 2, 0, done);
     return launch_resnorm_partial_ref(ctx, lv, lv.u, rhs, done);
@@ -388,7 +388,7 @@ void norm_final(mhs_ctx* ctx, const Level& lv, int l, long long n, int mode)
 void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool fuse_norm = false, bool cont = false)
 {
     Level& lv = Ls[l];
-    const void* rhs = (lv.dim == 3 && l == 0) ? nullptr : lv.rhs;
+    const void* rhs = lv.rhs /* (finest 3D level: NULL unless wall data is lifted into it) */;
     if (l >= clus_of(ctx, Ls) && !lv.coarsest && !cont) {   // this level and everything below it: one cluster-kernel launch
         Scope sc(ctx, kc_for(lv, l, 0));
         launch_cluster(ctx, Ls, l, l == 0 ? 1 : 0, done);
@@ -654,8 +654,15 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     if (o.dtype != MHS_F32 && o.dtype != MHS_F64) return fail(ctx, MHS_ERR_INVALID_ARG, "dtype must be MHS_F32 or MHS_F64");
     ctx->es = o.dtype == MHS_F64 ? 8 : 4;
     ctx->stream = (cudaStream_t)o.stream;
-    if (bc && (bc->sides != MHS_BC_DIRICHLET_ZERO || bc->top != MHS_BC_DIRICHLET_ZERO))
-        return fail(ctx, MHS_ERR_INVALID_ARG, "only MHS_BC_DIRICHLET_ZERO (P = 0 on sides and top, PAPER.md:96) is supported");
+    if (bc) {
+        for (int v : {bc->sides, bc->top})
+            if (v != MHS_BC_DIRICHLET_ZERO && v != MHS_BC_DIRICHLET_DATA)
+                return fail(ctx, MHS_ERR_INVALID_ARG, "mhs_bc: MHS_BC_DIRICHLET_ZERO (P = 0, PAPER.md:96) or MHS_BC_DIRICHLET_DATA (P given, mhs_set_wall_data)");
+        ctx->bc_sides = bc->sides; ctx->bc_top = bc->top;
+        ctx->wall_ctx = grid->nz > 1 && (bc->sides == MHS_BC_DIRICHLET_DATA || bc->top == MHS_BC_DIRICHLET_DATA);
+        if (ctx->wall_ctx && (ctx->opt.smoother != MHS_SMOOTH_JACOBI || ctx->opt.fmg_cycles != 0))
+            return fail(ctx, MHS_ERR_INVALID_ARG, "MHS_BC_DIRICHLET_DATA needs the point-Jacobi smoother and fmg_cycles = 0");
+    }
     if (!(o.omega > 0.0 && o.omega <= 1.0) || o.n_pre < 0 || o.n_post < 0 || o.n_pre + o.n_post < 1 || o.max_levels < 0 ||
         !(o.mu0 > 0.0) || o.g == 0.0 || o.boundary_max_cycles < 1 || !(grid->Lx > 0 && grid->Ly > 0 && grid->Lz > 0) ||
         (o.smoother != MHS_SMOOTH_JACOBI && o.smoother != MHS_SMOOTH_ZLINE) || o.fmg_cycles < 0)
@@ -723,6 +730,12 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
     if (!only2d) ctx->npartial = std::max(ctx->npartial, resnorm_partial_capacity(ctx->L3[0]));
     for (const Level& lv : ctx->L3) ctx->npartial = std::max(ctx->npartial, smooth_z_partial_capacity(ctx, lv));
     ctx->npartial = std::max<long long>(ctx->npartial, 4 * ctx->num_sms);
+    if (ctx->wall_ctx) {   // wall data W and a dense scratch copy of P for mhs_fields, both N elements, W = 0 until mhs_set_wall_data
+        const size_t nb = (size_t)ctx->L3[0].npts() * ctx->es;
+        CK(cudaMalloc(&ctx->wall, nb));
+        CK(cudaMemset(ctx->wall, 0, nb));
+        CK(cudaMalloc(&ctx->dense_P, nb));
+    }
     CK(cudaMalloc((void**)&ctx->partial, sizeof(double) * (size_t)ctx->npartial));
     CK(cudaMalloc((void**)&ctx->ctl, sizeof(Ctl)));
     CK(cudaMemset(ctx->ctl, 0, sizeof(Ctl)));
@@ -752,6 +765,8 @@ void mhs_destroy(mhs_ctx* ctx)
     if (ctx->ev_copied) cudaEventDestroy(ctx->ev_copied);
     if (ctx->stage) cudaFree(ctx->stage);
     if (ctx->bz_stage) cudaFree(ctx->bz_stage);
+    if (ctx->wall) cudaFree(ctx->wall);
+    if (ctx->dense_P) cudaFree(ctx->dense_P);
     for (const Ev& e : ctx->ev_pending) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (cudaEvent_t e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
@@ -921,6 +936,21 @@ mhs_status mhs_get_potential(mhs_ctx* ctx, void* P)
     if (!P) return fail(ctx, MHS_ERR_INVALID_ARG, "P is NULL");
     Scope sc(ctx, MHS_KC_PACK);
     launch_unpack(ctx, ctx->L3[0], ctx->L3[0].u, P);
+    if (ctx->wall_ctx) launch_wall_add(ctx, ctx->L3[0], ctx->wall, P);   // P = P_h + W
+    CK(cudaGetLastError());
+    return MHS_OK;
+}
+
+mhs_status mhs_set_wall_data(mhs_ctx* ctx, const void* G)
+{
+    if (!ctx) return MHS_ERR_INVALID_ARG;
+    if (!ctx->wall_ctx) return fail(ctx, MHS_ERR_STATE, "mhs_set_wall_data on a context created without MHS_BC_DIRICHLET_DATA");
+    if (!G) return fail(ctx, MHS_ERR_INVALID_ARG, "G is NULL");
+    Scope sc(ctx, MHS_KC_PACK);
+    Level& l0 = ctx->L3[0];
+    launch_wall_take(ctx, l0, ctx->bc_sides == MHS_BC_DIRICHLET_DATA, ctx->bc_top == MHS_BC_DIRICHLET_DATA, G, ctx->wall);
+    launch_wall_rhs(ctx, l0, ctx->wall, l0.rhs);   // (only interior nodes are written; the rest of rhs0 stays zero)
+    ctx->have_r0 = false;                          // r0 belongs to the problem: the next solve takes it afresh
     CK(cudaGetLastError());
     return MHS_OK;
 }
@@ -989,6 +1019,15 @@ mhs_status mhs_fields(mhs_ctx* ctx, void* B, void* p, void* rho)
     if (!B && !p && !rho) return MHS_OK;
     Scope sc(ctx, MHS_KC_FIELDS);
     const Level& l0 = ctx->L3[0];
+    if (ctx->wall_ctx) {
+        // the nodes next to a side or top wall take the wall values of P through the central differences: the general
+        // one-thread-per-node kernel on the dense P = P_h + W
+        launch_unpack(ctx, l0, l0.u, ctx->dense_P);
+        launch_wall_add(ctx, l0, ctx->wall, ctx->dense_P);
+        launch_fields_ref(ctx, l0, ctx->dense_P, B, p, rho, false, true);
+        CK(cudaGetLastError());
+        return MHS_OK;
+    }
     if (!(ctx->opt.flags & (MHS_FLAG_REFERENCE_KERNELS | MHS_FLAG_LOADED_FIELDS)) && launch_fields_ring(ctx, l0, l0.u, B, p, rho)) {
         ctx->prof.ring_fields += 1;
         launch_fields_ref(ctx, l0, l0.u, B, p, rho, true);
@@ -1181,7 +1220,7 @@ mhs_status mhs_op_residual(mhs_ctx* ctx, int dim, int level)
     Level& lv = (*Ls)[level];
     if (!lv.r) return fail(ctx, MHS_ERR_INVALID_ARG, "the coarsest level has no residual array");
     Scope sc(ctx, kc_for(lv, level, 1));
-    launch_residual_ref(ctx, lv, lv.u, (dim == 3 && level == 0) ? nullptr : lv.rhs, lv.r, nullptr);
+    launch_residual_ref(ctx, lv, lv.u, lv.rhs, lv.r, nullptr);
     CK(cudaGetLastError());
     return MHS_OK;
 }
@@ -1195,7 +1234,7 @@ mhs_status mhs_op_restrict(mhs_ctx* ctx, int dim, int level)
     Level& lv = (*Ls)[level];
     if (lv.coarsest) return fail(ctx, MHS_ERR_INVALID_ARG, "no level below the coarsest");
     Scope sc(ctx, kc_for(lv, level, 1));
-    const void* rhs = (dim == 3 && level == 0) ? nullptr : lv.rhs;
+    const void* rhs = lv.rhs;
     if (use_fast(ctx, lv)) {
         restrict_fast(ctx, lv, lv.u, rhs, (*Ls)[level + 1], 0, nullptr);
     } else {

@@ -80,6 +80,11 @@ struct mhs_ctx {
     cudaEvent_t ev_fields = nullptr, ev_copied = nullptr;
     bool copy_pending = false;
     bool have_boundary = false, have_r0 = false;
+    // Dirichlet data on the side / top faces (mhs_bc = MHS_BC_DIRICHLET_DATA; mhs_kernels_wall.cu): W = the data on the wall nodes,
+    // zero elsewhere (dense, N elements); the finest level then has a right-hand side (-L W); dense_P: N elements of scratch
+    bool wall_ctx = false;
+    int bc_sides = 0, bc_top = 0;
+    void *wall = nullptr, *dense_P = nullptr;
     bool fmg_pending = false;          // mhs_solve_boundary has run and no interior cycle yet: the FMG start may replace the interior
     const mhs::Level* ref_level = nullptr;   // a level that must run the general reference kernels right now (FMG start)
     double r0_interior = 0;
@@ -159,7 +164,12 @@ long long resnorm_partial_capacity(const Level& lv);
 void launch_norm_final(mhs_ctx* c, long long n, int mode);
 void launch_pack(mhs_ctx* c, const Level& lv, const void* dense, void* dst, bool keep_bottom, bool negate);
 void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense);
-void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only = false);
+// dense: P is a dense array (pitch nx, walls stored) instead of the level's aliased layout
+void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only = false, bool dense = false);
+// ---- Dirichlet data on the side / top faces (mhs_kernels_wall.cu) ----
+void launch_wall_take(mhs_ctx* c, const Level& lv, int sides, int top, const void* G, void* W);
+void launch_wall_rhs(mhs_ctx* c, const Level& lv, const void* W, void* rhs);
+void launch_wall_add(mhs_ctx* c, const Level& lv, const void* W, void* P);
 // ---- one-pass field recovery (mhs_kernels_fields.cu): planes 1 .. nz-2 ----
 bool fields_z_ok(const mhs_ctx* c, const Level& lv);
 void launch_fields_z(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho);

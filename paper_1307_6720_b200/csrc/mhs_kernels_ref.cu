@@ -358,10 +358,11 @@ void launch_unpack(mhs_ctx* c, const Level& lv, const void* src, void* dense)
 }
 
 template <typename T>
-static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only)
+static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only, bool dense)
 {
     FieldsP<T> q;
     q.nx = lv.nx; q.ny = lv.ny; q.nz = lv.nz; q.sx = lv.sx; q.sp = lv.sp;
+    if (dense) { q.sx = lv.nx; q.sp = (long long)lv.nx * lv.ny; }
     q.alpha = (T)c->alpha;
     q.i2hx = (T)(1.0 / (2.0 * lv.hx)); q.i2hy = (T)(1.0 / (2.0 * lv.hy)); q.i2hz = (T)(1.0 / (2.0 * lv.hz));
     q.ihx2 = (T)(1.0 / (lv.hx * lv.hx)); q.ihy2 = (T)(1.0 / (lv.hy * lv.hy));
@@ -376,11 +377,11 @@ static void fields_ref_t(mhs_ctx* c, const Level& lv, const void* P, void* B, vo
 }
 
 // ends_only: just the planes k = 0 and k = nz-1 (the rest is done by launch_fields_z)
-void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only)
+void launch_fields_ref(mhs_ctx* c, const Level& lv, const void* P, void* B, void* p, void* rho, bool ends_only, bool dense)
 {
     count_launch(c);
-    if (c->es == 8) fields_ref_t<double>(c, lv, P, B, p, rho, ends_only);
-    else fields_ref_t<float>(c, lv, P, B, p, rho, ends_only);
+    if (c->es == 8) fields_ref_t<double>(c, lv, P, B, p, rho, ends_only, dense);
+    else fields_ref_t<float>(c, lv, P, B, p, rho, ends_only, dense);
 }
 
 }  // namespace mhs

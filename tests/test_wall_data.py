@@ -74,3 +74,100 @@ def test_oracle_wall_data_is_linear_superposition(orc):
     sol = {k: orc.solve_interior(start(*k), w.f, w.alpha, w.L, tol=1e-13, max_cycles=80)[0] for k in ((1, 1), (1, 0), (0, 1))}
     assert np.abs(sol[(1, 1)] - sol[(1, 0)] - sol[(0, 1)]).max() <= 1e-10 * np.abs(sol[(1, 1)]).max()
     assert np.abs(sol[(0, 1)]).max() > 0.1 * np.abs(G).max()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# GPU: mhs_set_wall_data against the oracle
+# ------------------------------------------------------------------------------------------------------------------
+def _gpu_case(w, dtype, flags, orc, iterates=3):
+    import torch
+    from paper_1307_6720_b200 import binding
+    TOL = {torch.float64: 1e-12, torch.float32: 1e-5}[dtype]
+    G = inputs.wall_data(w)
+    if dtype == torch.float32:
+        G = G.astype(np.float32).astype(np.float64)          # both sides take the data the GPU can hold
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=dtype, device="cuda")
+    rel = lambda a, b: np.abs(a - b).max() / np.abs(b).max()
+    with binding.Solver.from_workload(w, dtype=dtype, flags=flags, bc=(binding.MHS_BC_DIRICHLET_DATA, binding.MHS_BC_DIRICHLET_DATA)) as S:
+        S.solve_boundary(dev(w.Bz0))
+        S.set_wall_data(dev(G))
+        P0 = S.get_boundary().cpu().double().numpy()
+        # the oracle's starting iterate: wall data on the sides and the top, the 2D solution on the bottom plane, zero inside
+        Po = G.copy()
+        Po[1:-1, 1:-1, 1:-1] = 0.0
+        Po[0, 1:-1, 1:-1] = P0[1:-1, 1:-1]
+        start = S.get_potential().cpu().double().numpy()
+        assert rel(start, Po) <= 1e-15 if dtype == torch.float64 else rel(start, Po) <= 1e-7
+        r0 = 0.0
+        for it in range(iterates):                                     # per iterate (C21)
+            info = S.solve_interior(1e-30, 1)
+            Po, oi = orc.solve_interior(Po, w.f, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=1e-30, max_cycles=1, r0=r0)
+            r0 = oi["r0"]
+            got = S.get_potential().cpu().double().numpy()
+            assert rel(got, Po) <= TOL, (it, rel(got, Po))
+            if it == 0:
+                assert abs(info["r0"] - r0) <= 50 * TOL * r0
+        # converged: restart from the 2D solution, solve to tolerance
+        S.solve_boundary(dev(w.Bz0))
+        tol = 1e-10 if dtype == torch.float64 else 1e-5
+        info = S.solve_interior(tol, 80)
+        Pc = G.copy(); Pc[1:-1, 1:-1, 1:-1] = 0.0; Pc[0, 1:-1, 1:-1] = P0[1:-1, 1:-1]
+        Pc, oc = orc.solve_interior(Pc, w.f, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=tol, max_cycles=80)
+        got = S.get_potential().cpu().double().numpy()
+        if dtype == torch.float64:
+            assert info["cycles"] == oc["cycles"]
+        assert rel(got, Pc) <= (TOL if dtype == torch.float64 else 20 * TOL)
+        assert np.abs(got[:, :, 0] - G[:, :, 0]).max() <= 1e-6 * np.abs(G).max() and np.abs(got[-1] - G[-1])[1:-1, 1:-1].max() <= 1e-6 * np.abs(G).max()
+        # fields of the full potential (the nodes next to the walls see the wall values)
+        Bf, p, rho = S.fields()
+        ref = orc.fields(got, w.f, w.alpha, w.L, w.p_b, w.rho_b, mu0=w.mu0, g=w.g)
+        FT = 1e-11 if dtype == torch.float64 else 2e-3
+        bmax = max(np.abs(ref[q]).max() for q in range(3))
+        for q in range(3):
+            assert np.abs(Bf[q].cpu().double().numpy() - ref[q]).max() <= FT * bmax, q
+        assert np.abs(p.cpu().double().numpy() - ref[3]).max() <= FT * np.abs(ref[3]).max()
+        if dtype == torch.float64:
+            assert np.abs(rho.cpu().double().numpy() - ref[4]).max() <= 1e-10 * np.abs(ref[4]).max()
+        return info
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("case", ["small_cluster", "cfg1_65_mid", "cfg1_65_big", "cfg1_65_big_sep", "small_ref"])
+@pytest.mark.parametrize("f32", [False, True])
+def test_wall_data_parity(orc, case, f32):
+    import torch
+    from paper_1307_6720_b200 import binding
+    w = inputs.small() if case.startswith("small") else inputs.config(1, shrink=2)
+    flags = {"small_cluster": 0, "cfg1_65_mid": 0, "cfg1_65_big": binding.MHS_FLAG_BIG_LEVEL_KERNELS,
+             "cfg1_65_big_sep": binding.MHS_FLAG_BIG_LEVEL_KERNELS | binding.MHS_FLAG_SEPARATE_PROLONG,
+             "small_ref": binding.MHS_FLAG_REFERENCE_KERNELS}[case]
+    _gpu_case(w, torch.float32 if f32 else torch.float64, flags, orc)
+
+
+@pytest.mark.gpu
+def test_wall_data_state_and_zero_data(orc):
+    """Without mhs_set_wall_data (or with zeros) a wall context returns what an ordinary context returns; the call is refused
+    on an ordinary context; one face may stay MHS_BC_DIRICHLET_ZERO."""
+    import torch
+    from paper_1307_6720_b200 import binding
+    w = inputs.small()
+    bz = torch.as_tensor(w.Bz0, device="cuda")
+    with binding.Solver.from_workload(w) as S:
+        S.solve_boundary(bz); S.solve_interior(1e-10, 60)
+        Pz = S.get_potential().cpu().numpy()
+        with pytest.raises(binding.MHSError) as e:
+            S.set_wall_data(torch.zeros(w.shape, dtype=torch.float64, device="cuda"))
+        assert e.value.status == binding.MHS_ERR_STATE
+    with binding.Solver.from_workload(w, bc=(1, 1)) as S:
+        S.solve_boundary(bz); S.solve_interior(1e-10, 60)
+        assert np.abs(S.get_potential().cpu().numpy() - Pz).max() <= 1e-12 * np.abs(Pz).max()
+    G = inputs.wall_data(w)
+    with binding.Solver.from_workload(w, bc=(0, 1)) as S:            # data on the top only: the side values of G are ignored
+        S.solve_boundary(bz); S.set_wall_data(torch.as_tensor(G, device="cuda")); S.solve_interior(1e-10, 80)
+        got = S.get_potential().cpu().numpy()
+    Po = np.zeros(w.shape); Po[-1, 1:-1, 1:-1] = G[-1, 1:-1, 1:-1]
+    P0, _ = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly)); Po[0] = P0
+    Po, _ = orc.solve_interior(Po, w.f, w.alpha, w.L, tol=1e-10, max_cycles=80)
+    assert np.abs(got - Po).max() <= 1e-12 * np.abs(Po).max()
+    with pytest.raises(binding.MHSError):
+        binding.Solver.from_workload(w, bc=(1, 1), smoother=binding.MHS_SMOOTH_ZLINE if hasattr(binding, "MHS_SMOOTH_ZLINE") else 1)
