@@ -718,6 +718,7 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ctx->debug = getenv("MHS_DEBUG") != nullptr;
         ctx->no_align = getenv("MHS_NO_ALIGN") != nullptr;
         if (const char* e = getenv("MHS_MID_PTS")) ctx->mid_pts = atoll(e);
+        if (const char* e = getenv("MHS_CL3_PTS")) ctx->cl3_pts = atoll(e);
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;
     const bool ref3 = ref || ctx->opt.smoother == MHS_SMOOTH_ZLINE;   // (the cluster kernel smooths with point Jacobi)

@@ -94,6 +94,7 @@ struct mhs_ctx {
     int device = 0;            // the CUDA device the context was created on
     bool debug = false;        // MHS_DEBUG was set at create: launch shapes go to stderr
     bool no_align = false;     // MHS_NO_ALIGN was set at create: k_zsweep keeps the cost-balanced ranges (A/B of the aligned z-segments)
+    long long cl3_pts = 0;     // levels of a big 3D hierarchy up to this many nodes run inside the cluster kernel (cluster_start(); knob MHS_CL3_PTS)
     long long mid_pts = 5000000;   // levels up to this many nodes are 'mid levels' (mid_level(); tuning knob MHS_MID_PTS, read at create)
     int tail3 = 1 << 30, tail2 = 1 << 30;  // first level kept in shared memory by the cluster kernel's CTA 0
     int clus3 = 1 << 30, clus2 = 1 << 30;  // first level handled by the cluster kernel (<= tail; mhs_kernels_cluster.cu)

@@ -739,7 +739,12 @@ int cluster_start(const mhs_ctx* c, const std::vector<Level>& Ls, int tail)
     if (tail >= n) return n;   // no tail -> no cluster kernel (the coarsest solve is part of the tail)
     // A hierarchy whose finest level is big keeps only the tail here: its middle levels (<= 129^3) fill the GPU
     // better as ordinary grids (mhs_kernels_fast.cu, mid_level) than on the 16 SMs of one cluster.
-    if (Ls[0].dim == 3 && (Ls[0].npts() > CL_MAX_PTS || (c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS))) return tail;
+    if (Ls[0].dim == 3 && (Ls[0].npts() > CL_MAX_PTS || (c->opt.flags & MHS_FLAG_BIG_LEVEL_KERNELS))) {
+        // (tuning knob MHS_CL3_PTS, read at create: levels of a big hierarchy up to that many nodes join the cluster kernel)
+        int l = tail;
+        while (l > 1 && tail - (l - 1) <= CL_MAXG && Ls[l - 1].npts() <= c->cl3_pts) --l;
+        return l;
+    }
     int l = tail;
     while (l > 0 && tail - (l - 1) <= CL_MAXG && Ls[l - 1].npts() <= CL_MAX_PTS && Ls[l - 1].sp < (1LL << 30) / std::max(1, Ls[l - 1].nz)) --l;
     return l;
