@@ -171,3 +171,41 @@ def test_wall_data_state_and_zero_data(orc):
     assert np.abs(got - Po).max() <= 1e-12 * np.abs(Po).max()
     with pytest.raises(binding.MHSError):
         binding.Solver.from_workload(w, bc=(1, 1), smoother=binding.MHS_SMOOTH_ZLINE if hasattr(binding, "MHS_SMOOTH_ZLINE") else 1)
+
+
+@pytest.mark.gpu
+def test_wall_data_from_elliptic_problems_on_the_other_faces(orc):
+    """PAPER.md:96 as a whole: "other elliptic equations ... on the other boundaries".  A Poisson problem (eq 11's kind) is
+    solved on the top face and on the two x-faces by boundary-only contexts (nz = 1), their solutions become the wall data of
+    the 3D solve; the oracle does the same with its 2D and 3D drivers.  Every face problem has P = 0 on its own edges, so the
+    faces agree along the edges of the box."""
+    import torch
+    from paper_1307_6720_b200 import binding
+    w = inputs.config(1, shrink=4)                                           # 33^3
+    nz, ny, nx = w.shape
+    rng = inputs.SplitMix64(inputs.SEED_BASE + 777)
+    faces = {"top": (nx, ny, w.Lx, w.Ly), "x0": (ny, nz, w.Ly, w.Lz), "x1": (ny, nz, w.Ly, w.Lz)}
+    G = np.zeros(w.shape)
+    Go = np.zeros(w.shape)
+    for name, (n1, n2, L1, L2) in faces.items():
+        src = inputs.random_patches(rng, 2, n1, n2, L1, L2, 0.1 * L1, 0.25 * L1)
+        with binding.Solver(n1, n2, 1, L=(L1, L2, 1.0)) as F:
+            F.solve_boundary(torch.as_tensor(src, device="cuda"))
+            sol = F.get_boundary().cpu().numpy()
+        solo, _ = orc.solve_boundary(src, (L1, L2))
+        assert np.abs(sol - solo).max() <= 1e-12 * np.abs(solo).max()
+        for arr, s in ((G, sol), (Go, solo)):
+            if name == "top": arr[nz - 1] = s
+            elif name == "x0": arr[:, :, 0] = s
+            else: arr[:, :, nx - 1] = s
+    with binding.Solver.from_workload(w, bc=(1, 1)) as S:
+        S.solve_boundary(torch.as_tensor(w.Bz0, device="cuda"))
+        S.set_wall_data(torch.as_tensor(G, device="cuda"))
+        info = S.solve_interior(1e-10, 80)
+        got = S.get_potential().cpu().numpy()
+    P0, _ = orc.solve_boundary(w.Bz0, (w.Lx, w.Ly))
+    Po = Go.copy(); Po[1:-1, 1:-1, 1:-1] = 0.0; Po[0, 1:-1, 1:-1] = P0[1:-1, 1:-1]
+    Po, oi = orc.solve_interior(Po, w.f, w.alpha, w.L, tol=1e-10, max_cycles=80)
+    assert info["cycles"] == oi["cycles"]
+    assert np.abs(got - Po).max() <= 1e-12 * np.abs(Po).max()
+    assert np.abs(got[nz - 1]).max() > 0 and np.abs(got[:, :, 0]).max() > 0
