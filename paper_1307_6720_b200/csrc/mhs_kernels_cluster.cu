@@ -343,11 +343,15 @@ struct Who { int wg, nW, lane; };
 
 template <typename T, bool D3>
 struct RowIt {     // iterates the interior row segments of a level
-    int xch, nitems, sy1;
-    __device__ RowIt(int sx, int sy, int nz) : xch((sx - 1 + 31) / 32), sy1(sy - 1) { nitems = sy1 * (D3 ? nz - 2 : 1) * xch; }
+    int xch, nitems, sy1, xsh;   // xsh: log2(xch) when the number of 32-node segments per row is a power of two (a shift instead of a division)
+    __device__ RowIt(int sx, int sy, int nz) : xch((sx - 1 + 31) / 32), sy1(sy - 1)
+    {
+        nitems = sy1 * (D3 ? nz - 2 : 1) * xch;
+        xsh = (xch & (xch - 1)) == 0 ? __ffs(xch) - 1 : -1;
+    }
     __device__ __forceinline__ bool at(int it, int lane, int sx, int sp, int& i, int& j, int& k, int& idx) const
     {
-        const int row = it / xch, c = it - row * xch;
+        const int row = xsh >= 0 ? it >> xsh : it / xch, c = it - row * xch;
         const int kk = D3 ? row / sy1 : 0, jj = row - kk * sy1;
         i = 1 + 32 * c + lane; j = jj + 1; k = D3 ? kk + 1 : 0;
         idx = i + sx * j + sp * k;
@@ -372,6 +376,20 @@ __device__ double ph_sweep(const GLevelP<T>& L, const T* __restrict__ u, const T
 {
     const RowIt<T, D3> R(L.sx, L.sy, L.nz);
     double acc = 0.0;
+    if (!D3) {   // one plane: the coefficients are three numbers, read once per phase instead of once per item
+        const T cx = L.tab[0], cy = L.tab[L.nz], wk = L.tab[3 * L.nz];
+#pragma unroll 4
+        for (int it = w.wg; it < R.nitems; it += w.nW) {
+            int i, j, k, idx;
+            if (!R.at(it, w.lane, L.sx, L.sp, i, j, k, idx)) continue;
+            const T f = rhs ? ldcg(rhs + idx) : T(0);
+            const T uc = ldcg(u + idx);
+            const T r = f - (cx * lap1<T>(ldcg(u + idx + 1), ldcg(u + idx - 1), uc) + cy * lap1<T>(ldcg(u + idx + L.sx), ldcg(u + idx - L.sx), uc));
+            out[idx] = uc + wk * r;
+            if (NORM) acc += (double)r * (double)r;
+        }
+        return acc;
+    }
 #pragma unroll 4
     for (int it = w.wg; it < R.nitems; it += w.nW) {
         int i, j, k, idx;
