@@ -86,6 +86,8 @@ typedef struct { int sides, top; } mhs_bc; /* the four side faces / the top face
                                         instead of the bulk-copy fed one; for A/B tests                         */
 #define MHS_FLAG_LOADED_FIELDS    128 /* mhs_fields by the register z-streaming kernel instead of the bulk-copy fed
                                         one; for A/B tests                                                      */
+#define MHS_FLAG_NO_FOLDED_NORM   256 /* keep the stop rule a kernel launch of its own instead of folding it into the finest
+                                        level's restriction kernel; for A/B tests                                    */
 #define MHS_FLAG_SYNC_EACH_CYCLE   2 /* read the norm back after every cycle instead of running
                                         cycles speculatively behind a device-side stop flag          */
 

@@ -26,6 +26,7 @@ MHS_FLAG_SEPARATE_PROLONG = 16
 MHS_FLAG_NO_PDL = 32
 MHS_FLAG_LOADED_RESTRICT = 64
 MHS_FLAG_LOADED_FIELDS = 128
+MHS_FLAG_NO_FOLDED_NORM = 256
 MHS_SMOOTH_JACOBI, MHS_SMOOTH_ZLINE = 0, 1
 MHS_HISTORY_LEN = 256
 MHS_KC_COUNT = 8

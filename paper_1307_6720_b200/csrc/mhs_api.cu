@@ -304,17 +304,37 @@ bool use_zsweep(const mhs_ctx* ctx, const Level& lv)
            !(ctx->opt.smoother == MHS_SMOOTH_ZLINE && lv.dim == 3);
 }
 
+// A stop rule that vcycle() left to the finest-level restriction and that kernel cannot take: as a launch of its own.
+void flush_pending_norm(mhs_ctx* ctx, const Level& lv)
+{
+    if (ctx->pending_norm <= 0) return;
+    const int prev = ctx->cur_kc;
+    ctx->cur_kc = lv.dim == 3 ? MHS_KC_NORM_L0 : prev;
+    launch_norm_final(ctx, ctx->pending_norm, 1);
+    ctx->cur_kc = prev;
+    ctx->pending_norm = 0;
+}
+
 // residual + full weighting into co.rhs: separable form on big levels, register z-streaming on the others
 void restrict_fast(mhs_ctx* ctx, const Level& lv, const void* u, const void* rhs, const Level& co, int reverse, const int* done)
 {
     if (!mid_level(ctx, lv) && !(ctx->opt.flags & MHS_FLAG_UNFUSED_KERNELS) && lv.nz >= 5) {
         // no right-hand side (the finest level): the bulk-copy fed kernel (walking down in z, to meet the planes the smoothing
         // pass wrote last while they are still in the L2, measured no different from walking up: 31.7 against 31.0 us at 257^3)
-        if (!rhs && !(ctx->opt.flags & MHS_FLAG_LOADED_RESTRICT) && launch_resid_restrict_ring(ctx, lv, u, co, co.rhs, 0, done)) return;
+        if (!rhs && !(ctx->opt.flags & MHS_FLAG_LOADED_RESTRICT)) {
+            const long long np = ctx->pending_norm;
+            if (launch_resid_restrict_ring(ctx, lv, u, co, co.rhs, 0, done, np)) { ctx->pending_norm = 0; return; }
+            if (np > 0) {    // could not be folded in after all: the stop rule as a launch of its own, then the restriction
+                flush_pending_norm(ctx, lv);
+                if (launch_resid_restrict_ring(ctx, lv, u, co, co.rhs, 0, done)) return;
+            }
+        }
+        flush_pending_norm(ctx, lv);
         launch_resid_restrict_sep(ctx, lv, u, rhs, co, co.rhs, reverse, done);
-    }
-    else
+    } else {
+        flush_pending_norm(ctx, lv);
         launch_resid_restrict_z(ctx, lv, u, rhs, co, co.rhs, reverse, done);
+    }
 }
 
 int clus_of(const mhs_ctx* ctx, const std::vector<Level>& Ls) { return Ls[0].dim == 3 ? ctx->clus3 : ctx->clus2; }
@@ -350,6 +370,13 @@ long long smooth(mhs_ctx* ctx, std::vector<Level>& Ls, int l, int sweeps, const 
     }
     for (int s = 0; s < sweeps; ++s) {
         Scope sc(ctx, kc_for(lv, l, 0));
+        if (fast && l > 0 && rhs && sweeps - s >= 2 && !(want_norm && s == 0) && smooth2_node_ok(ctx, lv) &&
+            !(ctx->opt.flags & MHS_FLAG_UNFUSED_KERNELS)) {
+            launch_smooth2_node(ctx, lv, lv.u, rhs, lv.tmp, done);      // two sweeps, one launch (small levels)
+            std::swap(lv.u, lv.tmp);
+            ++s;
+            continue;
+        }
         if (fast) {
             const long long n = launch_smooth_z(ctx, lv, lv.u, rhs, lv.tmp, (want_norm && s == 0) ? 1 : 0, ctx->dir, done);
             if (want_norm && s == 0) npart = n;
@@ -431,7 +458,11 @@ void vcycle(mhs_ctx* ctx, std::vector<Level>& Ls, int l, const int* done, bool f
         // norm; in the speculative units issued after that one it is skipped.  (Launched unconditionally it would, in those
         // later units and for an odd number of ping-pong passes per cycle, write into the buffer that holds the final iterate.)
         const long long np = smooth(ctx, Ls, l, first, done, true);
-        norm_final(ctx, lv, l, np, 1);
+        // The stop rule: a one-block kernel of its own -- or, when the restriction follows at once (no pre-smoothing pass
+        // left, which would overwrite the iterate) and is the bulk-copy fed kernel, folded into that kernel's CTA 0
+        // (restrict_fast): one dependent launch less per cycle, ~4 us at 257^3.
+        if (n_pre - first == 0 && fast && !rhs && ctx->opt.profile < 2 && !(ctx->opt.flags & MHS_FLAG_NO_FOLDED_NORM)) ctx->pending_norm = np;
+        else norm_final(ctx, lv, l, np, 1);
         smooth(ctx, Ls, l, n_pre - first, done);
     } else {
         smooth(ctx, Ls, l, n_pre, done);
@@ -718,6 +749,7 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ctx->debug = getenv("MHS_DEBUG") != nullptr;
         ctx->no_align = getenv("MHS_NO_ALIGN") != nullptr;
         if (const char* e = getenv("MHS_MID_PTS")) ctx->mid_pts = atoll(e);
+        if (const char* e = getenv("MHS_S2_PTS")) ctx->s2_pts = atoll(e);
         if (const char* e = getenv("MHS_CL3_PTS")) ctx->cl3_pts = atoll(e);
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;

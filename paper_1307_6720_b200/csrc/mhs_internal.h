@@ -95,11 +95,13 @@ struct mhs_ctx {
     bool debug = false;        // MHS_DEBUG was set at create: launch shapes go to stderr
     bool no_align = false;     // MHS_NO_ALIGN was set at create: k_zsweep keeps the cost-balanced ranges (A/B of the aligned z-segments)
     long long cl3_pts = 0;     // levels of a big 3D hierarchy up to this many nodes run inside the cluster kernel (cluster_start(); knob MHS_CL3_PTS)
+    long long s2_pts = 40000;   // levels up to this many nodes (33^3) smooth two sweeps per launch (k_smooth2_node; knob MHS_S2_PTS, 0 = off; measured at 257^3: off 3235, 40000: 3255, 300000: 3250 V-cycles/s)
     long long mid_pts = 5000000;   // levels up to this many nodes are 'mid levels' (mid_level(); tuning knob MHS_MID_PTS, read at create)
     int tail3 = 1 << 30, tail2 = 1 << 30;  // first level kept in shared memory by the cluster kernel's CTA 0
     int clus3 = 1 << 30, clus2 = 1 << 30;  // first level handled by the cluster kernel (<= tail; mhs_kernels_cluster.cu)
     int cluster_max = 8;                   // largest thread-block cluster the device co-schedules (<= 16)
     int dir = 0;               // z traversal direction of the next big kernel (alternates)
+    long long pending_norm = 0;   // partial sums of a norm whose stop rule the next finest-level restriction is to apply (vcycle)
     std::vector<mhs::Ev> ev_pending;
     std::vector<cudaEvent_t> ev_pool;
     std::string err;
@@ -194,12 +196,18 @@ bool mid_level(const mhs_ctx* c, const Level& lv);   // small enough to live in 
 long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done);
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);
+// two sweeps in one launch, one thread per node (levels up to c->s2_pts nodes with a right-hand side)
+bool smooth2_node_ok(const mhs_ctx* c, const Level& lv);
+void launch_smooth2_node(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done);
 void launch_resid_restrict_z(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
 // the same for a big level, in separable form (no plane of u kept, the residual never formed)
 void launch_resid_restrict_sep(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, int reverse, const int* done);
 // the same for a level WITHOUT a right-hand side (the finest 3D level), fed by the bulk-copy engine (mhs_kernels_restrict.cu);
 // down: walk down in z.  false: shape not supported, nothing launched.
-bool launch_resid_restrict_ring(mhs_ctx* c, const Level& fine, const void* u, const Level& coarse, void* rhs_c, int down, const int* done);
+// norm_n > 0: the cycle's stop rule (the reduction of c->partial[0 .. norm_n) and stop_rule, i.e. k_norm_final mode 1) is done by
+// CTA 0 of this kernel before its own work; false then also means "not folded in, nothing launched".
+bool launch_resid_restrict_ring(mhs_ctx* c, const Level& fine, const void* u, const Level& coarse, void* rhs_c, int down, const int* done,
+                                long long norm_n = 0);
 void launch_prolong_v(mhs_ctx* c, const Level& fine, void* u, const Level& coarse, const void* ec, int reverse, const int* done);
 // ---- temporally blocked smoother (mhs_kernels_zfused.cu) ----
 bool zsweep_ok(const mhs_ctx* c, const Level& lv);

@@ -409,6 +409,48 @@ long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv)
     return ((items + 127) / 128) * (long long)std::max(1, lv.nz - 2);   // (at most one z-chunk per plane)
 }
 
+// TWO Jacobi sweeps in one launch on the smallest grid-kernel level (33^3: up to c->s2_pts nodes), one thread per node: sweep 1 is
+// formed on the fly at the seven nodes sweep 2 reads (a wall neighbour keeps its value).  Seven times the arithmetic of a
+// sweep -- but on these levels a sweep kernel is ~4.5 us of launch and load latency whatever it computes, and the two
+// post-smoothing sweeps of a level were two dependent launches.  Same expressions as one sweep after the other.
+template <typename T>
+__global__ void __launch_bounds__(128) k_smooth2_node(LP<T> p, const T* __restrict__ u, const T* __restrict__ rhs, T* __restrict__ out,
+                                                      const int* __restrict__ done)
+{
+    pdl_enter();
+    if (done && *done) return;
+    const int i = 1 + (int)(blockIdx.x * blockDim.x + threadIdx.x);
+    const int j = 1 + (int)(blockIdx.y * blockDim.y + threadIdx.y);
+    const int k = 1 + (int)blockIdx.z;
+    if (i > p.nx - 2 || j > p.ny - 2) return;
+    const long long c = i + (long long)p.sx * j + p.sp * k;
+    auto sweep1 = [&](long long q, int kk, bool interior) -> T {
+        if (!interior) return u[q];     // a wall node passes through (zero, or the bottom data of a full-multigrid level)
+        return u[q] + p.tab[3 * p.nz + kk] * (rhs[q] - apply_L<T, true>(p, u, q, kk));
+    };
+    const T uc = sweep1(c, k, true);
+    const T e = sweep1(c + 1, k, i + 1 <= p.nx - 2), w = sweep1(c - 1, k, i - 1 >= 1);
+    const T n = sweep1(c + p.sx, k, j + 1 <= p.ny - 2), s = sweep1(c - p.sx, k, j - 1 >= 1);
+    const T up = sweep1(c + p.sp, k + 1, k + 1 <= p.nz - 2), dn = sweep1(c - p.sp, k - 1, k - 1 >= 1);
+    const T lu = p.tab[k] * lap1<T>(e, w, uc) + p.tab[p.nz + k] * lap1<T>(n, s, uc) + p.cz * lap1<T>(up, dn, uc) + p.a2 * uc;
+    out[c] = uc + p.tab[3 * p.nz + k] * (rhs[c] - lu);
+}
+
+bool smooth2_node_ok(const mhs_ctx* c, const Level& lv)
+{
+    return lv.dim == 3 && lv.nz >= 3 && lv.rhs && lv.npts() <= c->s2_pts && fast_ok(c, lv);
+}
+
+void launch_smooth2_node(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done)
+{
+    static PerDevice once;
+    per_device(once, c, [&] { prefer_l1(k_smooth2_node<double>); prefer_l1(k_smooth2_node<float>); return 1; });
+    count_launch(c);
+    const dim3 block(32, 4), grid((unsigned)((lv.nx - 2 + 31) / 32), (unsigned)((lv.ny - 2 + 3) / 4), (unsigned)(lv.nz - 2));
+    if (c->es == 8) launch_pdl(c, k_smooth2_node<double>, grid, block, 0, lp_of<double>(c, lv), (const double*)u, (const double*)rhs, (double*)out, done);
+    else launch_pdl(c, k_smooth2_node<float>, grid, block, 0, lp_of<float>(c, lv), (const float*)u, (const float*)rhs, (float*)out, done);
+}
+
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done)
 {
     static PerDevice once;

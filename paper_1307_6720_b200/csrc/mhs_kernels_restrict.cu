@@ -82,6 +82,11 @@ struct RRP {
     int nring;                 // planes of the ring
     int ntiles, nzc;           // strips along y, z-chunks
     int down;                  // walk down in z
+    // The cycle's stop rule folded in (instead of a k_norm_final launch between the norm-carrying smoothing pass and this
+    // kernel): CTA 0 reduces the norm_n partial sums of the squared residual and applies the rule before its own work.
+    const double* norm_partial;
+    long long norm_n;          // 0: nothing folded in
+    Ctl* ctl;
 };
 
 // One CTA: strip `tile` (coarse rows J0 .. J0+RC*G-1), coarse planes [Kb, Ke).
@@ -92,6 +97,25 @@ __global__ void __launch_bounds__(512, 1) k_resid_restrict_ring(const __grid_con
     constexpr int RC = RR_RC;
     constexpr int NROW = 2 * RC + 3;                       // fine rows under a thread's RC coarse rows
     pdl_enter();
+    if (p.norm_n > 0 && blockIdx.x == 0 && !p.ctl->done) {
+        // k_norm_final's reduction, sum for sum (1024 virtual threads q, q + 1024, ...; warp sums; their sum in warp 0), so the
+        // norms are the same bits whichever kernel forms them.  Every thread has read `done` before thread 0 may raise it
+        // (the barrier below).  The other CTAs do not wait for the decision: in the one cycle that finds the tolerance met
+        // they restrict a residual nobody uses; every later kernel of that cycle sees the flag.
+        __shared__ double s_vw[32];
+        for (int t = (int)threadIdx.x; t < 1024; t += (int)blockDim.x) {
+            double v = 0.0;
+            for (long long q = t; q < p.norm_n; q += 1024) v += p.norm_partial[q];
+            v = warp_sum(v);
+            if ((t & 31) == 0) s_vw[t >> 5] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            const double w = warp_sum(s_vw[threadIdx.x]);
+            if (threadIdx.x == 0) stop_rule(p.ctl, sqrt(w), 1);
+        }
+        __syncthreads();
+    }
     if (done && *done) return;
     extern __shared__ __align__(128) unsigned char rsm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(rsm);
@@ -213,7 +237,7 @@ __global__ void __launch_bounds__(512, 1) k_resid_restrict_ring(const __grid_con
 }
 
 template <typename T>
-bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void* rc, int down, const int* done)
+bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void* rc, int down, const int* done, long long norm_n)
 {
     constexpr int RC = RR_RC;
     const int ncx = f.sx / 2;
@@ -247,6 +271,8 @@ bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void*
     // z-chunks: one CTA per SM, no chunk shorter than 4 coarse planes (2 n + 3 fine planes are read for n)
     p.nzc = std::max(1, std::min(planes / 4 > 0 ? planes / 4 : 1, c->num_sms * MHS_RR_CPS / p.ntiles));
     p.down = down;
+    p.norm_partial = c->partial; p.norm_n = norm_n; p.ctl = c->ctl;
+    if (norm_n > 0 && ((ncx * G) % 32 || !done)) return false;         // (the folded reduction works on whole warps)
     const size_t smem = 128 + (size_t)nring * (2 * RC * G + 3) * f.sx * sizeof(T) + 16;   // (+ the element after the last row)
     launch_pdl(c, kern, dim3((unsigned)(p.ntiles * p.nzc)), dim3((unsigned)(ncx * G)), smem, p, (const T*)u, (T*)rc, done);
     return true;
@@ -256,10 +282,10 @@ bool rr_launch(mhs_ctx* c, const Level& f, const void* u, const Level& co, void*
 
 // rhs_c <- R (0 - L u) on a level without a right-hand side (the finest 3D level); false: not launched (shape not
 // supported), the caller takes k_resid_restrict_sep.
-bool launch_resid_restrict_ring(mhs_ctx* c, const Level& f, const void* u, const Level& co, void* rc, int down, const int* done)
+bool launch_resid_restrict_ring(mhs_ctx* c, const Level& f, const void* u, const Level& co, void* rc, int down, const int* done, long long norm_n)
 {
     if (f.dim != 3 || f.nz < 5) return false;
-    const bool ok = c->es == 8 ? rr_launch<double>(c, f, u, co, rc, down, done) : rr_launch<float>(c, f, u, co, rc, down, done);
+    const bool ok = c->es == 8 ? rr_launch<double>(c, f, u, co, rc, down, done, norm_n) : rr_launch<float>(c, f, u, co, rc, down, done, norm_n);
     if (ok) { count_launch(c); c->prof.ring_restrict += 1; }
     return ok;
 }

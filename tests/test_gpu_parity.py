@@ -470,6 +470,36 @@ def test_dependent_launch_is_invisible(B, name):
                 assert torch.equal(Bf, ref[key][1]), (name, rep, flags)
 
 
+@pytest.mark.parametrize("name", ["cfg1_65", "cfg1_129", "ragged_25x49x13"])
+@pytest.mark.parametrize("sweeps", [(2, 2), (1, 1), (3, 2)])
+def test_folded_stop_rule_is_invisible(B, name, sweeps):
+    """The cycle's stop rule is applied by CTA 0 of the finest level's restriction kernel when that kernel follows the
+    norm-carrying pass at once (V(2,2), V(1,1): folded; V(3,2): a pre-smoothing pass is left, not folded) instead of by a
+    kernel launch of its own (MHS_FLAG_NO_FOLDED_NORM).  Same reduction, sum for sum: iterate, cycle count AND the residual
+    history must be bitwise the same either way, on the big-level kernels (where the fold applies) and on the default ones."""
+    w = WORKLOADS[name]()
+    dt = torch.float64 if w.dtype == "f64" else torch.float32
+    for big in (B.MHS_FLAG_BIG_LEVEL_KERNELS, 0):
+        res = []
+        for flags in (big, big | B.MHS_FLAG_NO_FOLDED_NORM, big | B.MHS_FLAG_SYNC_EACH_CYCLE):
+            with B.Solver.from_workload(w, flags=flags, n_pre=sweeps[0], n_post=sweeps[1]) as S:
+                S.solve_boundary(dev(w.Bz0, dt))
+                ii = S.solve_interior(w.tol, w.max_cycles)
+                res.append((S.get_potential().clone(), ii, S.profile()))
+        for q, (P, ii, prof) in enumerate(res[1:]):
+            assert ii["cycles"] == res[0][1]["cycles"]
+            if q == 0:      # folded against not folded: the norms themselves, bit for bit
+                assert ii["r0"] == res[0][1]["r0"] and np.array_equal(ii["history"], res[0][1]["history"])
+            else:           # (a whole solve in one cluster-kernel launch sums its norm in another order than the per-cycle path)
+                assert abs(ii["r0"] - res[0][1]["r0"]) <= 1e-12 * ii["r0"]
+                assert np.allclose(ii["history"], res[0][1]["history"], rtol=1e-12, atol=0)
+            assert torch.equal(P, res[0][0])
+        if big and sweeps != (3, 2) and res[0][2]["ring_restrict"] > 0 and not name.startswith("ragged"):
+            # the fold really happened (the ragged grid's restriction kernel has 12-column thread groups: its block is not made
+            # of whole warps, the fold is refused and the launch of its own comes back -- that path is covered too)
+            assert res[0][2]["launches"]["norm_l0"] < res[1][2]["launches"]["norm_l0"]
+
+
 def test_full_size_per_iterate_parity(B, orc):
     """BASELINE configs[2] at FULL size (257^3 fp64) in the launch configuration bench.py times (default flags:
     temporally blocked finest level, fine-grained mid levels, shared-memory tail): the first V-cycle iterates are
