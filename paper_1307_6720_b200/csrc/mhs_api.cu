@@ -333,7 +333,8 @@ void restrict_fast(mhs_ctx* ctx, const Level& lv, const void* u, const void* rhs
         launch_resid_restrict_sep(ctx, lv, u, rhs, co, co.rhs, reverse, done);
     } else {
         flush_pending_norm(ctx, lv);
-        launch_resid_restrict_z(ctx, lv, u, rhs, co, co.rhs, reverse, done);
+        if (rhs && !(ctx->opt.flags & MHS_FLAG_UNFUSED_KERNELS) && resid_restrict_box_ok(ctx, lv)) launch_resid_restrict_box(ctx, lv, u, rhs, co, co.rhs, done);
+        else launch_resid_restrict_z(ctx, lv, u, rhs, co, co.rhs, reverse, done);
     }
 }
 
@@ -750,6 +751,7 @@ mhs_status mhs_create(const mhs_grid* grid, double alpha, const double* f_profil
         ctx->no_align = getenv("MHS_NO_ALIGN") != nullptr;
         if (const char* e = getenv("MHS_MID_PTS")) ctx->mid_pts = atoll(e);
         if (const char* e = getenv("MHS_S2_PTS")) ctx->s2_pts = atoll(e);
+        if (const char* e = getenv("MHS_RB_PTS")) ctx->rb_pts = atoll(e);
         if (const char* e = getenv("MHS_CL3_PTS")) ctx->cl3_pts = atoll(e);
     }
     const bool ref = (ctx->opt.flags & MHS_FLAG_REFERENCE_KERNELS) != 0;

@@ -95,6 +95,7 @@ struct mhs_ctx {
     bool debug = false;        // MHS_DEBUG was set at create: launch shapes go to stderr
     bool no_align = false;     // MHS_NO_ALIGN was set at create: k_zsweep keeps the cost-balanced ranges (A/B of the aligned z-segments)
     long long cl3_pts = 0;     // levels of a big 3D hierarchy up to this many nodes run inside the cluster kernel (cluster_start(); knob MHS_CL3_PTS)
+    long long rb_pts = 40000;   // levels up to this many nodes restrict with the box kernel (k_resid_restrict_box; knob MHS_RB_PTS, 0 = off)
     long long s2_pts = 40000;   // levels up to this many nodes (33^3) smooth two sweeps per launch (k_smooth2_node; knob MHS_S2_PTS, 0 = off; measured at 257^3: off 3235, 40000: 3255, 300000: 3250 V-cycles/s)
     long long mid_pts = 5000000;   // levels up to this many nodes are 'mid levels' (mid_level(); tuning knob MHS_MID_PTS, read at create)
     int tail3 = 1 << 30, tail2 = 1 << 30;  // first level kept in shared memory by the cluster kernel's CTA 0
@@ -196,6 +197,9 @@ bool mid_level(const mhs_ctx* c, const Level& lv);   // small enough to live in 
 long long launch_smooth_z(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, int mode, int reverse, const int* done);
 long long smooth_z_partial_capacity(const mhs_ctx* c, const Level& lv);
 void launch_scale_rhs(mhs_ctx* c, const Level& lv, const void* rhs, void* u, const int* done);
+// residual + full weighting as a box kernel (levels up to c->rb_pts nodes with a right-hand side)
+bool resid_restrict_box_ok(const mhs_ctx* c, const Level& fine);
+void launch_resid_restrict_box(mhs_ctx* c, const Level& fine, const void* u, const void* rhs, const Level& coarse, void* rhs_c, const int* done);
 // two sweeps in one launch, one thread per node (levels up to c->s2_pts nodes with a right-hand side)
 bool smooth2_node_ok(const mhs_ctx* c, const Level& lv);
 void launch_smooth2_node(mhs_ctx* c, const Level& lv, const void* u, const void* rhs, void* out, const int* done);
