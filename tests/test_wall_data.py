@@ -209,3 +209,27 @@ def test_wall_data_from_elliptic_problems_on_the_other_faces(orc):
     assert info["cycles"] == oi["cycles"]
     assert np.abs(got - Po).max() <= 1e-12 * np.abs(Po).max()
     assert np.abs(got[nz - 1]).max() > 0 and np.abs(got[:, :, 0]).max() > 0
+
+
+@pytest.mark.gpu
+def test_wall_data_full_size_first_iterates(orc):
+    """BASELINE configs[2] at full size (257^3 fp64, default flags) with wall data: the finest level then runs the temporally
+    blocked smoother in its right-hand-side variants (with the norm by-product, with the prolongation folded in) and the
+    separable restriction with a right-hand side, in the launch shapes of the big grid.  Two iterates against the oracle."""
+    import torch
+    from paper_1307_6720_b200 import binding
+    w = inputs.config(2)
+    G = inputs.wall_data(w, amp=0.05)
+    with binding.Solver.from_workload(w, bc=(1, 1)) as S:
+        S.solve_boundary(torch.as_tensor(w.Bz0, device="cuda"))
+        S.set_wall_data(torch.as_tensor(G, device="cuda"))
+        P0 = S.get_boundary().cpu().numpy()
+        Po = G.copy(); Po[1:-1, 1:-1, 1:-1] = 0.0; Po[0, 1:-1, 1:-1] = P0[1:-1, 1:-1]
+        r0 = 0.0
+        for it in range(2):
+            S.solve_interior(1e-30, 1)
+            Po, oi = orc.solve_interior(Po, w.f, w.alpha, w.L, omega=w.omega, n_pre=w.n_pre, n_post=w.n_post, tol=1e-30, max_cycles=1, r0=r0)
+            r0 = oi["r0"]
+            got = S.get_potential().cpu().numpy()
+            assert np.abs(got - Po).max() <= 1e-12 * np.abs(Po).max(), it
+        assert S.profile()["sweeps_l0"] > 0
